@@ -1,0 +1,126 @@
+/* flashvan.h -- C-ABI of libflashvan.so: the B200 (sm_100a) hot path of FlashVAN
+ * (arxiv/paper_2606_22984): KV-cached ancestral sampling under a per-site CSR attention
+ * mask, the teacher-forced log q(s) pass, and the batched Ising energy.
+ *
+ * Citations are PAPER.md line + the section / equation / algorithm the line falls in.
+ * Readings of silent or garbled passages are numbered A1..A21 in DESIGN.md.
+ *
+ * General rules
+ *   - Every array argument marked [device] is a CUDA device pointer allocated by the caller
+ *     and borrowed for the call; arguments marked [host] are host pointers.  The library
+ *     never frees caller memory.  fv_create_model copies what it keeps.
+ *   - `stream` is a cudaStream_t passed as void*.  fv_sample, fv_log_prob, fv_energy_* and
+ *     fv_free_energy only enqueue work on it and never synchronise the device;
+ *     fv_create_model / fv_destroy_model synchronise.
+ *   - Return value: 0 on success, a negative FV_ERR_* otherwise; fv_last_error() then gives a
+ *     thread-local message.  Outputs are unspecified after an error.  There is no CPU
+ *     fallback and no other backend: a non-sm_100 device is FV_ERR_ARCH.
+ *   - Results are bit-reproducible run to run for fixed inputs (no float atomics).
+ *   - 0-based positions.  Position t takes the token of spin t-1 (start token 0 for t = 0,
+ *     sharing id 0 with spin -1) and emits the conditional of spin t (PAPER.md:314-363,
+ *     Alg. 2 l.6-11; reading A3).
+ */
+#ifndef FLASHVAN_H
+#define FLASHVAN_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FV_OK 0
+#define FV_ERR_BAD_ARG (-1)   /* NULL pointer, non-positive size, B > max_batch            */
+#define FV_ERR_BAD_MASK (-2)  /* row not ascending/unique, col > row, col < 0, last != row  */
+#define FV_ERR_BAD_SHAPE (-3) /* unsupported d_model / head size / n_weights mismatch       */
+#define FV_ERR_CUDA (-4)      /* a CUDA runtime call failed                                 */
+#define FV_ERR_OOM (-5)       /* device allocation failed                                   */
+#define FV_ERR_ARCH (-6)      /* current device is not compute capability 10.x              */
+
+typedef struct fv_model fv_model; /* opaque, library-owned */
+
+/* Architecture of the decoder (PAPER.md:92-109 II.A.3; Alg. 1 l.226-246; Alg. 2 l.314-363). */
+typedef struct {
+    int32_t n_sites;   /* N: sequence length = number of spins                               */
+    int32_t n_layers;  /* n_l decoder layers                                                 */
+    int32_t d_model;   /* d = d_token + d_pos (Eq. 15 l.287-292); 32, 64, 128 or 256          */
+    int32_t n_heads;   /* n_h; d_h = d / n_h must be 8, 16, 32 or 64                          */
+    int32_t d_token;   /* token-embedding width (paper default 2, l.577)                     */
+    int32_t ffn_mult;  /* FFN hidden width / d; must be 4 (pinned by the paper's counts, P1)  */
+    int32_t has_wo;    /* 0: W_O bypassed as in the paper (l.107); 1: u <- W_O u + b_O        */
+    int32_t act;       /* 0: exact GELU (reading A5); no other value is defined               */
+    int32_t ln2_style; /* 0: h += FFN(LN2(h)) (Alg. 2 l.346); 1: h = LN2(h); h += FFN(h)      */
+                       /*    (Alg. 1 l.237-239); reading A1                                   */
+    int32_t max_batch; /* KV pool is sized for this many samples                              */
+    int32_t kv_page;   /* positions per KV page (power of two >= 8); 0 selects 64             */
+    float ln_eps;      /* LayerNorm epsilon (reading A6: 1e-5)                                */
+} fv_config;
+
+/* Build a model object.
+ *   weights [host]  n_weights fp32 values in this order, matrices row-major [out,in], y = Wx+b
+ *       (Eq. 2, l.98-100): tok_emb[2,d_token]; per layer ln1_g[d] ln1_b[d] Wq[d,d] bq[d]
+ *       Wk[d,d] bk[d] Wv[d,d] bv[d] (Wo[d,d] bo[d] iff has_wo) ln2_g[d] ln2_b[d] W1[4d,d]
+ *       b1[4d] W2[d,4d] b2[d]; then head_W[2,d] head_b[2].  GEMM operands are rounded to bf16
+ *       once here; LayerNorm, biases, embeddings and the head stay fp32.
+ *   mask_rowptr [host] N+1, mask_col [host] rowptr[N]: CSR in POSITION space (reading A11):
+ *       row t lists the key positions A(t), ascending, unique, all <= t, last entry == t
+ *       (Eq. 3 l.102 sums j <= t; Eq. S1 l.555 is the banded special case).
+ *   posemb [host] [N, d_model - d_token] fp32 (Eq. 15).
+ * Allocates the paged bf16 KV pool: max_batch * n_layers * N rows of 2d bf16 (K then V).
+ * Synchronises `stream`.  *out is owned by the library until fv_destroy_model. */
+int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weights,
+                    const int32_t* mask_rowptr, const int32_t* mask_col, const float* posemb,
+                    void* stream, fv_model** out);
+
+/* Alg. 2: ancestral sampling of B <= max_batch configurations.
+ *   uniforms [device] [B,N] fp32 in [0,1): spin t of sample b is +1 iff u[b,t] < p_t(+1)
+ *       (strict, compared in fp32; reading A10 replaces Categorical(p_t), l.359).
+ *   spins  [device] [B,N] int8 out, values +-1 (l.361: sigma = 2 s - 1).
+ *   logq   [device] [B] fp32 out: sum_t log p_t(s_t) (Alg. 1 l.9), accumulated in fp64.
+ *   cond_p [device] [B,N] fp32 out or NULL: p_t(+1 | s_<t). */
+int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, float* logq,
+              float* cond_p, void* stream);
+
+/* Alg. 1: teacher-forced log q(s) of given configurations.
+ *   spins [device] [B,N] int8 in (+-1; other values are undefined behaviour).
+ *   logq, cond_p as in fv_sample.  Overwrites the model's KV pool. */
+int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p,
+                void* stream);
+
+/* Eq. 8: E_b = - sum over listed bonds J_ij s_i s_j, every bond listed once.
+ *   rowptr [device] N+1, col [device], val [device] fp32: CSR of the bonds (any triangle).
+ *   integer_couplings != 0: every val is an integer; the sum is taken in int32 and is exact.
+ *   E [device] [B] fp32 out. */
+int fv_energy_csr(int32_t B, int32_t N, const int8_t* spins, const int32_t* rowptr,
+                  const int32_t* col, const float* val, int32_t integer_couplings, float* E,
+                  void* stream);
+
+/* Eq. 6 (1/sqrt(N) folded into J; reading A15): E_b = - sum_{i<j} J_ij s_i s_j
+ * = -1/2 s^T J s for symmetric J with zero diagonal.
+ *   J [device] [N,N] fp32 row-major, symmetric, zero diagonal.  E [device] [B] fp32 out. */
+int fv_energy_dense(int32_t B, int32_t N, const int8_t* spins, const float* J, float* E,
+                    void* stream);
+
+/* Eq. 5: L_b = E_b + T logq_b; out[0] = mean_b L_b, out[1] = population std.
+ *   E, logq [device] [B] fp32; out [device] 2 x fp64.  Deterministic single-block fp64 tree. */
+int fv_free_energy(int32_t B, const float* E, const float* logq, double temperature, double* out,
+                   void* stream);
+
+void fv_destroy_model(fv_model* m);
+
+/* Expected n_weights for a configuration (the layout above); < 0 on a bad shape. */
+int64_t fv_n_weights(const fv_config* cfg);
+
+/* Bytes of device memory the model's KV pool occupies (0 for NULL). */
+int64_t fv_kv_bytes(const fv_model* m);
+
+/* Number of kernel launches the library has enqueued since load (for bench.py gpu_launches). */
+int64_t fv_launch_count(void);
+
+/* Thread-local message of the last failing call; valid until the next call on the thread. */
+const char* fv_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLASHVAN_H */

@@ -1,0 +1,182 @@
+"""Thin ctypes binding over libflashvan.so (include/flashvan.h) -- argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; torch is used for device
+memory and streams.  There is no CPU fallback: if the library is missing or the device is not
+a B200-class GPU the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libflashvan.so")
+
+SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
+           "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
+           "fv_last_error"]
+
+
+class FvConfig(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in
+                ("n_sites", "n_layers", "d_model", "n_heads", "d_token", "ffn_mult", "has_wo", "act",
+                 "ln2_style", "max_batch", "kv_page")] + [("ln_eps", ctypes.c_float)]
+
+
+class FlashVanError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libflashvan.so (built in-tree by build.py / __graft_entry__.build()); fail loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise FlashVanError(f"{_LIB_PATH} is missing: run `python -m paper_2606_22984_b200.build` "
+                                "(there is no CPU fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        L.fv_create_model.argtypes = [ctypes.POINTER(FvConfig), vp, i64, vp, vp, vp, vp, ctypes.POINTER(vp)]
+        L.fv_sample.argtypes = [vp, i32, vp, vp, vp, vp, vp]
+        L.fv_log_prob.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.fv_energy_csr.argtypes = [i32, i32, vp, vp, vp, vp, i32, vp, vp]
+        L.fv_energy_dense.argtypes = [i32, i32, vp, vp, vp, vp]
+        L.fv_free_energy.argtypes = [i32, vp, vp, ctypes.c_double, vp, vp]
+        L.fv_destroy_model.argtypes = [vp]
+        L.fv_destroy_model.restype = None
+        L.fv_n_weights.argtypes = [ctypes.POINTER(FvConfig)]
+        L.fv_n_weights.restype = i64
+        L.fv_kv_bytes.argtypes = [vp]
+        L.fv_kv_bytes.restype = i64
+        L.fv_launch_count.restype = i64
+        L.fv_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise FlashVanError(f"{what} failed ({rc}): {lib().fv_last_error().decode()}")
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dev(t: torch.Tensor, dtype) -> torch.Tensor:
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise FlashVanError(f"expected a contiguous CUDA tensor of {dtype}, got {t.dtype} on {t.device}")
+    return t
+
+
+def launch_count() -> int:
+    return int(lib().fv_launch_count())
+
+
+def make_config(w, max_batch: int, kv_page: int = 64) -> FvConfig:
+    """`w` is any object with the Workload fields (n_sites, n_layers, d_model, ...)."""
+    return FvConfig(w.n_sites, w.n_layers, w.d_model, w.n_heads, w.d_token, w.ffn_mult, w.has_wo, 0,
+                    w.ln2_style, max_batch, kv_page, float(w.ln_eps))
+
+
+class Model:
+    """Owner of an `fv_model*`.  create_model / sample / log_prob mirror the C entry points."""
+
+    def __init__(self, cfg: FvConfig, weights, mask_rowptr, mask_col, posemb):
+        weights = np.ascontiguousarray(weights, np.float32)
+        rp = np.ascontiguousarray(mask_rowptr, np.int32)
+        col = np.ascontiguousarray(mask_col, np.int32)
+        pe = np.ascontiguousarray(posemb, np.float32)
+        if rp.size != cfg.n_sites + 1 or pe.size != cfg.n_sites * (cfg.d_model - cfg.d_token):
+            raise FlashVanError("mask_rowptr / posemb size does not match the configuration")
+        if col.size != int(rp[-1]):
+            raise FlashVanError("mask_col size != mask_rowptr[N]")
+        self.cfg = cfg
+        self._h = ctypes.c_void_p()
+        torch.cuda.init()
+        _check(lib().fv_create_model(ctypes.byref(cfg), weights.ctypes.data, weights.size, rp.ctypes.data,
+                                     col.ctypes.data, pe.ctypes.data, _stream(), ctypes.byref(self._h)),
+               "fv_create_model")
+
+    @property
+    def kv_bytes(self) -> int:
+        return int(lib().fv_kv_bytes(self._h))
+
+    def sample(self, uniforms: torch.Tensor, want_cond_p: bool = False, out=None):
+        """fv_sample: uniforms [B,N] f32 cuda -> (spins int8 [B,N], logq f32 [B], cond_p or None)."""
+        u = _dev(uniforms, torch.float32)
+        B, N = u.shape
+        if N != self.cfg.n_sites:
+            raise FlashVanError("uniforms must be [B, n_sites]")
+        if out is None:
+            spins = torch.empty((B, N), dtype=torch.int8, device=u.device)
+            logq = torch.empty((B,), dtype=torch.float32, device=u.device)
+        else:
+            spins, logq = out
+        cp = torch.empty((B, N), dtype=torch.float32, device=u.device) if want_cond_p else None
+        _check(lib().fv_sample(self._h, B, u.data_ptr(), spins.data_ptr(), logq.data_ptr(),
+                               cp.data_ptr() if cp is not None else None, _stream()), "fv_sample")
+        return spins, logq, cp
+
+    def log_prob(self, spins: torch.Tensor, want_cond_p: bool = False, out=None):
+        """fv_log_prob: spins int8 [B,N] cuda -> (logq f32 [B], cond_p or None)."""
+        s = _dev(spins, torch.int8)
+        B, N = s.shape
+        if N != self.cfg.n_sites:
+            raise FlashVanError("spins must be [B, n_sites]")
+        logq = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+        cp = torch.empty((B, N), dtype=torch.float32, device=s.device) if want_cond_p else None
+        _check(lib().fv_log_prob(self._h, B, s.data_ptr(), logq.data_ptr(),
+                                 cp.data_ptr() if cp is not None else None, _stream()), "fv_log_prob")
+        return logq, cp
+
+    def close(self):
+        if self._h:
+            lib().fv_destroy_model(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def create_model(w, weights, mask_rowptr, mask_col, posemb, max_batch: int) -> Model:
+    return Model(make_config(w, max_batch), weights, mask_rowptr, mask_col, posemb)
+
+
+def energy_csr(spins, rowptr, col, val, integer_couplings: bool, out=None):
+    s = _dev(spins, torch.int8)
+    B, N = s.shape
+    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+    _check(lib().fv_energy_csr(B, N, s.data_ptr(), _dev(rowptr, torch.int32).data_ptr(),
+                               _dev(col, torch.int32).data_ptr(), _dev(val, torch.float32).data_ptr(),
+                               1 if integer_couplings else 0, E.data_ptr(), _stream()), "fv_energy_csr")
+    return E
+
+
+def energy_dense(spins, J, out=None):
+    s = _dev(spins, torch.int8)
+    B, N = s.shape
+    J = _dev(J, torch.float32)
+    if tuple(J.shape) != (N, N):
+        raise FlashVanError("J must be [N, N]")
+    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+    _check(lib().fv_energy_dense(B, N, s.data_ptr(), J.data_ptr(), E.data_ptr(), _stream()), "fv_energy_dense")
+    return E
+
+
+def free_energy(E, logq, temperature: float, out=None):
+    """fv_free_energy: returns a 2-element f64 CUDA tensor (mean, std of E + T log q)."""
+    E, logq = _dev(E, torch.float32), _dev(logq, torch.float32)
+    res = torch.empty((2,), dtype=torch.float64, device=E.device) if out is None else out
+    _check(lib().fv_free_energy(E.numel(), E.data_ptr(), logq.data_ptr(), float(temperature),
+                                res.data_ptr(), _stream()), "fv_free_energy")
+    return res

@@ -1,0 +1,299 @@
+// fv_api.cu -- the extern "C" boundary of libflashvan.so (see include/flashvan.h).
+// Host orchestration only: argument validation, one-off weight packing, launch geometry.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/flashvan.h"
+#include "fv_internal.h"
+
+struct fv_model {
+    fv_config cfg;
+    FvModelDev dev;
+    void* arena = nullptr;       // all read-only parameters, one allocation
+    size_t arena_bytes = 0;
+    size_t kv_bytes = 0;
+    int n_sms = 0;
+    int device = 0;
+};
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+    return fail(e == cudaErrorMemoryAllocation ? FV_ERR_OOM : FV_ERR_CUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+bool shape_ok(const fv_config* c) {
+    if (!c || c->n_sites <= 0 || c->n_layers <= 0 || c->n_layers > FV_MAX_LAYERS) return false;
+    if (c->ffn_mult != 4 || c->act != 0) return false;
+    if (c->d_token <= 0 || c->d_token >= c->d_model) return false;
+    if (c->n_heads <= 0 || c->d_model % c->n_heads) return false;
+    const int dh = c->d_model / c->n_heads;
+    const int key = c->d_model * 1000 + dh;
+    return key == 32016 || key == 64016 || key == 64032 || key == 128016 || key == 128032 || key == 256064;
+}
+
+int64_t n_weights_of(const fv_config* c) {
+    const int64_t d = c->d_model, f = 4 * d;
+    const int64_t per = 2 * d + 3 * (d * d + d) + (c->has_wo ? d * d + d : 0) + 2 * d + f * d + f + d * f + d;
+    return 2 * (int64_t)c->d_token + c->n_layers * per + 2 * d + 2;
+}
+
+uint16_t bf16_bits(float x) {
+    __nv_bfloat16 h = __float2bfloat16_rn(x);
+    uint16_t u;
+    std::memcpy(&u, &h, 2);
+    return u;
+}
+
+// W[out,in] fp32 row-major -> bf16 in mma.m16n8k16 A-fragment order: tile (mt,kt), lane, 8 values
+//   reg j/2: a0=(g, 2c..2c+1) a1=(g+8, 2c..) a2=(g, 2c+8..) a3=(g+8, 2c+8..),  g = lane/4, c = lane%4.
+void pack_mma_a(const float* W, int out, int in, uint16_t* dst) {
+    const int MT = out / 16, KT = in / 16;
+    for (int mt = 0; mt < MT; ++mt)
+        for (int kt = 0; kt < KT; ++kt)
+            for (int lane = 0; lane < 32; ++lane)
+                for (int j = 0; j < 8; ++j) {
+                    const int reg = j >> 1, half = j & 1, g = lane >> 2, c = lane & 3;
+                    const int row = mt * 16 + g + ((reg & 1) ? 8 : 0);
+                    const int k = kt * 16 + 2 * c + half + ((reg & 2) ? 8 : 0);
+                    dst[(((size_t)mt * KT + kt) * 32 + lane) * 8 + j] = bf16_bits(W[(size_t)row * in + k]);
+                }
+}
+
+struct Arena {
+    std::vector<unsigned char> host;
+    size_t reserve(size_t bytes) {
+        const size_t off = (host.size() + 255) / 256 * 256;
+        host.resize(off + bytes);
+        return off;
+    }
+    size_t put(const void* src, size_t bytes) {
+        const size_t off = reserve(bytes);
+        std::memcpy(host.data() + off, src, bytes);
+        return off;
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+const char* fv_last_error(void) { return g_err.c_str(); }
+int64_t fv_launch_count(void) { return g_launches.load(); }
+int64_t fv_n_weights(const fv_config* cfg) { return shape_ok(cfg) ? n_weights_of(cfg) : -1; }
+int64_t fv_kv_bytes(const fv_model* m) { return m ? (int64_t)m->kv_bytes : 0; }
+
+int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weights, const int32_t* mask_rowptr,
+                    const int32_t* mask_col, const float* posemb, void* stream, fv_model** out) {
+    if (!cfg || !weights || !mask_rowptr || !mask_col || !posemb || !out) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (!shape_ok(cfg)) return fail(FV_ERR_BAD_SHAPE, "unsupported d_model / n_heads / ffn_mult / act / n_layers");
+    if (cfg->max_batch <= 0) return fail(FV_ERR_BAD_ARG, "max_batch must be positive");
+    if (cfg->kv_page != 0 && (cfg->kv_page < 8 || (cfg->kv_page & (cfg->kv_page - 1))))
+        return fail(FV_ERR_BAD_ARG, "kv_page must be 0 or a power of two >= 8");
+    if (n_weights != n_weights_of(cfg)) return fail(FV_ERR_BAD_SHAPE, "n_weights does not match the configuration");
+    const int N = cfg->n_sites, d = cfg->d_model, f = 4 * d, NL = cfg->n_layers;
+    // mask validation (reading A11): ascending, unique, 0 <= col <= row, last entry == row
+    if (mask_rowptr[0] != 0) return fail(FV_ERR_BAD_MASK, "rowptr[0] != 0");
+    for (int t = 0; t < N; ++t) {
+        const int e0 = mask_rowptr[t], e1 = mask_rowptr[t + 1];
+        if (e1 <= e0) return fail(FV_ERR_BAD_MASK, "empty mask row " + std::to_string(t));
+        for (int e = e0; e < e1; ++e) {
+            if (mask_col[e] < 0 || mask_col[e] > t) return fail(FV_ERR_BAD_MASK, "col out of [0,row] in row " + std::to_string(t));
+            if (e > e0 && mask_col[e] <= mask_col[e - 1]) return fail(FV_ERR_BAD_MASK, "row not ascending/unique: " + std::to_string(t));
+        }
+        if (mask_col[e1 - 1] != t) return fail(FV_ERR_BAD_MASK, "row must end with itself: " + std::to_string(t));
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDeviceProperties");
+    if (prop.major != 10) return fail(FV_ERR_ARCH, "device is not compute capability 10.x (sm_100a required)");
+
+    fv_model* m = new fv_model();
+    m->cfg = *cfg;
+    m->n_sms = prop.multiProcessorCount;
+    m->device = dev;
+    Arena A;
+    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b; };
+    std::vector<Off> off(NL);
+    const float* w = weights;
+    const size_t o_tok = A.put(w, sizeof(float) * 2 * cfg->d_token);
+    w += 2 * cfg->d_token;
+    std::vector<uint16_t> pk((size_t)f * d);
+    std::vector<float> tmp((size_t)3 * d * d), tb(3 * d);
+    for (int l = 0; l < NL; ++l) {
+        Off& o = off[l];
+        o.ln1g = A.put(w, 4 * d); w += d;
+        o.ln1b = A.put(w, 4 * d); w += d;
+        for (int p = 0; p < 3; ++p) {             // Wq,bq,Wk,bk,Wv,bv -> one [3d,d] matrix + [3d] bias
+            std::memcpy(tmp.data() + (size_t)p * d * d, w, sizeof(float) * d * d); w += (size_t)d * d;
+            std::memcpy(tb.data() + p * d, w, sizeof(float) * d); w += d;
+        }
+        pack_mma_a(tmp.data(), 3 * d, d, pk.data());
+        o.wqkv = A.put(pk.data(), (size_t)3 * d * d * 2);
+        o.bqkv = A.put(tb.data(), 4 * 3 * d);
+        o.wo = o.bo = 0;
+        if (cfg->has_wo) {
+            pack_mma_a(w, d, d, pk.data()); w += (size_t)d * d;
+            o.wo = A.put(pk.data(), (size_t)d * d * 2);
+            o.bo = A.put(w, 4 * d); w += d;
+        }
+        o.ln2g = A.put(w, 4 * d); w += d;
+        o.ln2b = A.put(w, 4 * d); w += d;
+        pack_mma_a(w, f, d, pk.data()); w += (size_t)f * d;
+        o.w1 = A.put(pk.data(), (size_t)f * d * 2);
+        o.b1 = A.put(w, 4 * f); w += f;
+        pack_mma_a(w, d, f, pk.data()); w += (size_t)d * f;
+        o.w2 = A.put(pk.data(), (size_t)d * f * 2);
+        o.b2 = A.put(w, 4 * d); w += d;
+    }
+    std::vector<float> wd(d);
+    for (int i = 0; i < d; ++i) wd[i] = w[d + i] - w[i];            // head_W[1] - head_W[0]
+    const float bd = w[2 * d + 1] - w[2 * d];
+    const size_t o_wd = A.put(wd.data(), 4 * d);
+    const size_t o_pos = A.put(posemb, sizeof(float) * (size_t)N * (d - cfg->d_token));
+    const size_t o_rp = A.put(mask_rowptr, sizeof(int32_t) * (N + 1));
+    const size_t o_col = A.put(mask_col, sizeof(int32_t) * (size_t)mask_rowptr[N]);
+
+    m->arena_bytes = A.host.size();
+    e = cudaMalloc(&m->arena, m->arena_bytes);
+    if (e != cudaSuccess) { delete m; return cuda_fail(e, "cudaMalloc(parameters)"); }
+    m->kv_bytes = (size_t)cfg->max_batch * NL * N * 2 * d * sizeof(__nv_bfloat16);
+    void* kv = nullptr;
+    e = cudaMalloc(&kv, m->kv_bytes);
+    if (e != cudaSuccess) { cudaFree(m->arena); delete m; return cuda_fail(e, "cudaMalloc(KV pool)"); }
+    cudaStream_t s = (cudaStream_t)stream;
+    e = cudaMemcpyAsync(m->arena, A.host.data(), m->arena_bytes, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cudaFree(kv); cudaFree(m->arena); delete m; return cuda_fail(e, "parameter upload"); }
+
+    unsigned char* base = (unsigned char*)m->arena;
+    FvModelDev& D = m->dev;
+    D.n_sites = N; D.n_layers = NL; D.has_wo = cfg->has_wo; D.ln2_style = cfg->ln2_style;
+    D.ln_eps = cfg->ln_eps; D.d_token = cfg->d_token;
+    D.tok_emb = (const float*)(base + o_tok);
+    D.posemb = (const float*)(base + o_pos);
+    D.head_wd = (const float*)(base + o_wd);
+    D.head_bd = bd;
+    D.mask_rowptr = (const int32_t*)(base + o_rp);
+    D.mask_col = (const int32_t*)(base + o_col);
+    D.kv = (__nv_bfloat16*)kv;
+    for (int l = 0; l < NL; ++l) {
+        const Off& o = off[l];
+        FvLayerDev& L = D.layer[l];
+        L.wqkv = (const uint4*)(base + o.wqkv);
+        L.wo = cfg->has_wo ? (const uint4*)(base + o.wo) : nullptr;
+        L.w1 = (const uint4*)(base + o.w1);
+        L.w2 = (const uint4*)(base + o.w2);
+        L.bqkv = (const float*)(base + o.bqkv);
+        L.bo = cfg->has_wo ? (const float*)(base + o.bo) : nullptr;
+        L.b1 = (const float*)(base + o.b1);
+        L.b2 = (const float*)(base + o.b2);
+        L.ln1_g = (const float*)(base + o.ln1g); L.ln1_b = (const float*)(base + o.ln1b);
+        L.ln2_g = (const float*)(base + o.ln2g); L.ln2_b = (const float*)(base + o.ln2b);
+    }
+    *out = m;
+    return FV_OK;
+}
+
+void fv_destroy_model(fv_model* m) {
+    if (!m) return;
+    cudaDeviceSynchronize();
+    cudaFree(m->dev.kv);
+    cudaFree(m->arena);
+    delete m;
+}
+
+// Launch geometry of the persistent forward kernel.
+// SAMPLE: one CTA per SM; B samples are cut into groups of S <= 32 so that the number of groups
+// is (a multiple of) the SM count; NT = ceil(S/8) rounded to {1,2,4} n8-tiles per mma.
+static void sample_geometry(int B, int n_sms, int* S, int* nt, int* n_groups, int* grid) {
+    const int rounds = (B + n_sms * 32 - 1) / (n_sms * 32);
+    const int target = rounds * n_sms;
+    int s = (B + target - 1) / target;
+    if (s < 1) s = 1;
+    *nt = s <= 8 ? 1 : (s <= 16 ? 2 : 4);
+    *S = s;
+    *n_groups = (B + s - 1) / s;
+    *grid = *n_groups < n_sms ? *n_groups : n_sms;
+}
+
+int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, float* logq, float* cond_p,
+              void* stream) {
+    if (!m || !uniforms || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
+    FvForwardArgs a{};
+    a.mode = FV_MODE_SAMPLE;
+    a.B = B;
+    int nt, grid;
+    sample_geometry(B, m->n_sms, &a.rows_per_group, &nt, &a.n_groups, &grid);
+    a.uniforms = uniforms; a.spins_out = spins; a.logq = logq; a.cond_p = cond_p;
+    cudaError_t e = fv_launch_forward(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, grid,
+                                      (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_sample launch");
+    g_launches++;
+    return FV_OK;
+}
+
+int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {
+    if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
+    FvForwardArgs a{};
+    a.mode = FV_MODE_LOGPROB;
+    a.B = B;
+    a.samples_per_cta = (B + m->n_sms - 1) / m->n_sms;
+    const int grid = (B + a.samples_per_cta - 1) / a.samples_per_cta;
+    a.spins_in = spins; a.logq = logq; a.cond_p = cond_p;
+    // small tiles when a CTA owns very few rows, else 32-row tiles (least weight traffic per row)
+    const long long rows = (long long)a.samples_per_cta * m->cfg.n_sites;
+    const int nt = rows <= 8 ? 1 : (rows <= 16 ? 2 : 4);
+    cudaError_t e = fv_launch_forward(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, grid,
+                                      (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_log_prob launch");
+    g_launches++;
+    return FV_OK;
+}
+
+int fv_energy_csr(int32_t B, int32_t N, const int8_t* spins, const int32_t* rowptr, const int32_t* col,
+                  const float* val, int32_t integer_couplings, float* E, void* stream) {
+    if (!spins || !rowptr || !col || !val || !E) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || N <= 0) return fail(FV_ERR_BAD_ARG, "B and N must be positive");
+    cudaError_t e = fv_launch_energy_csr(B, N, spins, rowptr, col, val, integer_couplings, E, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_energy_csr launch");
+    g_launches++;
+    return FV_OK;
+}
+
+int fv_energy_dense(int32_t B, int32_t N, const int8_t* spins, const float* J, float* E, void* stream) {
+    if (!spins || !J || !E) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || N <= 0) return fail(FV_ERR_BAD_ARG, "B and N must be positive");
+    cudaError_t e = fv_launch_energy_dense(B, N, spins, J, E, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_energy_dense launch");
+    g_launches++;
+    return FV_OK;
+}
+
+int fv_free_energy(int32_t B, const float* E, const float* logq, double temperature, double* out, void* stream) {
+    if (!E || !logq || !out) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0) return fail(FV_ERR_BAD_ARG, "B must be positive");
+    cudaError_t e = fv_launch_free_energy(B, E, logq, temperature, out, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_free_energy launch");
+    g_launches++;
+    return FV_OK;
+}
+
+}  // extern "C"

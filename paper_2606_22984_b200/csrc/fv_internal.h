@@ -1,0 +1,60 @@
+// fv_internal.h -- shared declarations of the CUDA path (not part of the public ABI).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define FV_MAX_LAYERS 16
+
+// Per-layer device pointers.  GEMM weights are bf16, pre-packed at fv_create_model time into
+// mma.m16n8k16 A-fragment order: tile (mt, kt) of W[out,in] is 32 lanes x 16 B, contiguous,
+// so one warp-wide 128-bit load fetches a whole 16x16 tile (see pack_mma_a in fv_api.cu).
+struct FvLayerDev {
+    const uint4* wqkv;  // [3d, d]  rows: Wq, Wk, Wv            (Eq. 2)
+    const uint4* wo;    // [d, d] or nullptr                    (l.107: bypassed in the paper)
+    const uint4* w1;    // [4d, d]
+    const uint4* w2;    // [d, 4d]
+    const float *bqkv, *bo, *b1, *b2;
+    const float *ln1_g, *ln1_b, *ln2_g, *ln2_b;
+};
+
+struct FvModelDev {
+    int32_t n_sites, n_layers, has_wo, ln2_style;
+    float ln_eps;
+    int32_t d_token;
+    const float* tok_emb;   // [2, d_token]
+    const float* posemb;    // [N, d - d_token]
+    const float* head_wd;   // [d]  = head_W[1] - head_W[0]   (softmax over 2 logits == sigmoid)
+    float head_bd;          //      = head_b[1] - head_b[0]
+    const int32_t* mask_rowptr;
+    const int32_t* mask_col;
+    __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16)
+    FvLayerDev layer[FV_MAX_LAYERS];
+};
+
+enum { FV_MODE_SAMPLE = 0, FV_MODE_LOGPROB = 1 };
+
+struct FvForwardArgs {
+    int32_t mode;
+    int32_t B;
+    int32_t rows_per_group;      // SAMPLE: samples per group (<= 8*NT)
+    int32_t n_groups;            // SAMPLE: number of sample groups
+    int32_t samples_per_cta;     // LOGPROB: contiguous samples owned by one CTA
+    const float* uniforms;       // SAMPLE
+    const int8_t* spins_in;      // LOGPROB
+    int8_t* spins_out;           // SAMPLE
+    float* logq;
+    float* cond_p;               // may be nullptr
+};
+
+// Launchers (fv_forward.cu / fv_energy.cu).  Return cudaError_t of the launch.
+cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int nt,
+                              const FvForwardArgs& a, int grid, cudaStream_t s);
+size_t fv_forward_smem_bytes(int d_model, int nt);
+cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_t* rowptr,
+                                 const int32_t* col, const float* val, int integer, float* E,
+                                 cudaStream_t s);
+cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const float* J, float* E,
+                                   cudaStream_t s);
+cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out,
+                                  cudaStream_t s);

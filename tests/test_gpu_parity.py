@@ -1,0 +1,158 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by
+element, on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  * per-site conditionals within 2e-3 absolute (bf16 GEMM operands, bf16 KV cache);
+  * sampled spins identical to (u < p_oracle) except where |u - p_oracle| < 2e-3 (counted);
+  * +-J energies bit-exact, Gaussian energies within 1e-4 relative (to max(|E|, rms scale)).
+"""
+import dataclasses
+import itertools
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2606_22984_b200 import binding as fv
+from paper_2606_22984_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL_P = 2e-3
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def build(w, max_batch, weights=None, posemb=None, mask=None):
+    weights = W.make_weights(w) if weights is None else weights
+    posemb = W.make_posemb(w) if posemb is None else posemb
+    rp, col = W.make_mask_csr(w) if mask is None else mask
+    model = fv.create_model(w, weights, rp, col, posemb, max_batch)
+    return model, weights, posemb, rp, col
+
+
+def check_log_prob(w, model, weights, posemb, rp, col, spins, tol=TOL_P):
+    lq_o, cp_o = O.log_prob(w, weights, posemb, rp, col, spins)
+    lq_g, cp_g = model.log_prob(dev(spins), want_cond_p=True)
+    cp_g, lq_g = cp_g.cpu().numpy().astype(np.float64), lq_g.cpu().numpy().astype(np.float64)
+    assert np.isfinite(cp_g).all() and np.isfinite(lq_g).all()
+    dp = np.abs(cp_g - cp_o).max()
+    assert dp <= tol, f"max |dp| = {dp}"
+    picked = np.where(spins > 0, cp_o, 1 - cp_o)
+    bound = tol * (1.0 / picked).sum(1) + 1e-4 * np.abs(lq_o)        # first-order bound
+    assert (np.abs(lq_g - lq_o) <= bound).all(), np.abs(lq_g - lq_o).max()
+    return dp
+
+
+def check_sample(w, model, weights, posemb, rp, col, u, tol=TOL_P):
+    spins_g, lq_g, cp_g = model.sample(dev(u), want_cond_p=True)
+    spins_g = spins_g.cpu().numpy()
+    cp_g = cp_g.cpu().numpy().astype(np.float64)
+    lq_g = lq_g.cpu().numpy().astype(np.float64)
+    assert set(np.unique(spins_g)) <= {-1, 1}
+    lq_o, cp_o = O.log_prob(w, weights, posemb, rp, col, spins_g)     # re-synchronised on the GPU's spins
+    assert np.abs(cp_g - cp_o).max() <= tol, np.abs(cp_g - cp_o).max()
+    want = np.where(u.astype(np.float64) < cp_o, 1, -1)
+    mism = spins_g != want
+    tie = np.abs(u.astype(np.float64) - cp_o) < tol
+    assert not (mism & ~tie).any(), f"{(mism & ~tie).sum()} flips outside the tie band"
+    assert np.array_equal(spins_g, np.where(u < cp_g.astype(np.float32), 1, -1))   # its own draw rule
+    picked = np.where(spins_g > 0, cp_o, 1 - cp_o)
+    bound = tol * (1.0 / picked).sum(1) + 1e-4 * np.abs(lq_o)
+    assert (np.abs(lq_g - lq_o) <= bound).all()
+    # chain rule on the GPU: teacher-forced pass over its own samples reproduces its log q
+    lq_tf, cp_tf = model.log_prob(dev(spins_g), want_cond_p=True)
+    assert np.abs(cp_tf.cpu().numpy() - cp_g).max() <= 2e-4
+    assert np.abs(lq_tf.cpu().numpy() - lq_g).max() <= 2e-4 * max(1.0, np.abs(lq_g).max())
+    return int(tie.sum()), int(mism.sum())
+
+
+# --------------------------------------------------------------------------- cfg1 (full size)
+def test_cfg1_full_enumeration_normalised():
+    w = W.CONFIGS["cfg1"]
+    S = np.array(list(itertools.product([-1, 1], repeat=w.n_sites)), dtype=np.int8)
+    model, weights, posemb, rp, col = build(w, len(S))
+    lq_g, _ = model.log_prob(dev(S))
+    total = np.exp(lq_g.cpu().numpy().astype(np.float64)).sum()
+    assert abs(total - 1.0) < 1e-3, total
+    idx = np.arange(0, len(S), 61)
+    check_log_prob(w, model, weights, posemb, rp, col, S[idx])
+
+
+def test_cfg1_sample_full_batch():
+    w = W.CONFIGS["cfg1"]
+    model, weights, posemb, rp, col = build(w, w.batch)
+    ties, flips = check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w))
+    print(f"cfg1: near-tie sites {ties}, flips among them {flips}")
+
+
+# ----------------------------------------------- reduced cfg2..cfg5 (several tiles + ragged tail)
+CASES = {
+    "cfg2_small": (dict(L=8, n_sites=64, window=8), 75),
+    "cfg2_full_N": (dict(), 37),
+    "cfg3_small": (dict(L=100, n_sites=100), 41),
+    "cfg4_small": (dict(L=5, n_sites=125, window=16), 150),
+    "cfg5_small": (dict(L=12, n_sites=144, window=12), 19),
+    "cfg5_L16": (dict(L=16, n_sites=256, window=16, n_layers=6), 300),
+}
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_reduced_configs(case):
+    kw, B = CASES[case]
+    w = dataclasses.replace(W.CONFIGS[case.split("_")[0]], **kw)
+    model, weights, posemb, rp, col = build(w, B)
+    check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B))
+    ties, flips = check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B))
+    print(f"{case}: near-tie sites {ties}, flips among them {flips}")
+
+
+@pytest.mark.parametrize("variant", [dict(has_wo=1), dict(ln2_style=1), dict(n_heads=1, d_model=32),
+                                     dict(d_model=128, n_heads=4), dict(d_model=256, n_heads=4)])
+def test_variants(variant):
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2, **variant)
+    if w.d_model // w.n_heads not in (16, 32, 64) or (w.d_model, w.d_model // w.n_heads) == (32, 32):
+        pytest.skip("head size not instantiated")
+    B = 45
+    model, weights, posemb, rp, col = build(w, B)
+    check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B))
+    check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B))
+
+
+def test_sharp_conditionals_stress():
+    """head_W x40: p reaches the log-sigmoid tails; p tolerance scales with it."""
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=8, n_sites=64, window=8)
+    weights = W.make_weights(w, head_scale=40.0)
+    model, weights, posemb, rp, col = build(w, 64, weights=weights)
+    spins = W.make_spins(w, 64)
+    lq_o, cp_o = O.log_prob(w, weights, posemb, rp, col, spins)
+    lq_g, cp_g = model.log_prob(dev(spins), want_cond_p=True)
+    cp_g, lq_g = cp_g.cpu().numpy().astype(np.float64), lq_g.cpu().numpy().astype(np.float64)
+    assert np.isfinite(lq_g).all() and np.isfinite(cp_g).all()
+    assert min(cp_o.min(), 1 - cp_o.max()) < 0.05                       # the tails are exercised
+    assert np.abs(cp_g - cp_o).max() <= 40 * TOL_P
+    own = np.log(np.where(spins > 0, cp_g, 1 - cp_g)).sum(1)
+    assert np.abs(own - lq_g).max() <= 1e-4 * np.abs(lq_g).max() + 1e-3
+    assert np.abs(lq_g - lq_o).max() <= 40 * TOL_P * (1 / np.where(spins > 0, cp_o, 1 - cp_o)).sum(1).max()
+
+
+def test_batch_edges_and_errors():
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=4, n_sites=16, window=3, n_layers=2)
+    model, weights, posemb, rp, col = build(w, 200)
+    for B in (1, 7, 8, 9, 149, 200):                                     # ragged groups and tiles
+        check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=B))
+        check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=B))
+    with pytest.raises(fv.FlashVanError):
+        model.sample(dev(W.make_uniforms(w, 201)))
+    bad_col = col.copy()
+    bad_col[rp[5]] = 9                                                   # look-ahead entry in row 5
+    with pytest.raises(fv.FlashVanError, match="mask|row|col"):
+        fv.create_model(w, weights, rp, bad_col, posemb, 4)
+    with pytest.raises(fv.FlashVanError):
+        fv.create_model(dataclasses.replace(w, d_model=48, n_heads=3), weights, rp, col, posemb, 4)
+    # deterministic: two runs are bit-identical
+    u = dev(W.make_uniforms(w, 64))
+    a = model.sample(u, want_cond_p=True)
+    b = model.sample(u, want_cond_p=True)
+    assert all(torch.equal(x, y) for x, y in zip(a, b))
