@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- full-config samples/sec (with log q) of the FlashVAN hot path on B200.
+
+One "step" = one pass of the whole hot path over one batch of the workload:
+    fv_sample (Alg. 2)  ->  fv_log_prob (Alg. 1)  ->  fv_energy_*  ->  fv_free_energy (Eq. 5)
+`value` = samples/s with the uniforms already resident in HBM; `e2e` = the same through the
+public binding with HOST buffers (pinned uniforms in, spins/logq/E/F out) inside the timed region.
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_22984_b200 import workloads as W  # noqa: E402
+
+METRIC = "full-config samples/sec (with log q)"
+UNIT = "samples/s"
+
+
+def parse():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=3)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--workload", default="cfg5", choices=list(W.CONFIGS))
+    p.add_argument("--batch", type=int, default=0, help="override the workload's batch (debug only)")
+    p.add_argument("--cpu-samples", type=int, default=0, help="oracle samples for cpu_baseline (0 = 2 x cores)")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    return p.parse_args()
+
+
+def algorithmic_kv_bytes_per_sample(w, rowptr):
+    """KV rows named by the mask only: read sum_t nnz(t) rows + write N rows,
+    each 2d bf16 = 4d bytes, per layer."""
+    row_bytes = 4 * w.d_model
+    return int(rowptr[-1]) * w.n_layers * row_bytes, w.n_sites * w.n_layers * row_bytes
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        rows = [l.split(", ") for t, l in self.lines if t0 <= t <= t1] or [l.split(", ") for _, l in self.lines[-3:]]
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.strip().lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_step(w, inp, n):
+    """The oracle as it stands on n samples of the workload: sample + log_prob + energy + F_q."""
+    from oracle import oracle as O
+    u = inp["uniforms"][:n]
+    spins, lq, _ = O.sample(w, inp["weights"], inp["posemb"], inp["mask_rowptr"], inp["mask_col"], u)
+    lq2, _ = O.log_prob(w, inp["weights"], inp["posemb"], inp["mask_rowptr"], inp["mask_col"], spins)
+    if w.model == "sk":
+        E = O.energy_dense(spins, inp["J"])
+    else:
+        E = O.energy_csr(spins, inp["bond_rowptr"], inp["bond_col"], inp["bond_val"])
+    return O.free_energy(E, lq2, w.betas[0])
+
+
+def config_of(w, B, n_gpus):
+    return {"workload": f"{w.name}: {'SK' if w.model == 'sk' else str(w.dim) + 'D EA L=' + str(w.L)} N={w.n_sites}, "
+                        f"{w.n_layers} layers, d={w.d_model}, {w.n_heads} heads, {w.coupling} couplings, "
+                        f"mask window {w.window}", "batch_per_gpu": B, "global_batch": B * n_gpus,
+            "n_sites": w.n_sites, "parallelism": f"dp{n_gpus} (independent sample shards, no data-path collective)",
+            "l2_policy": "inputs_exceed_l2 (KV pool >> 126 MB; uniforms/spins rewritten every step)"}
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    w = W.CONFIGS[args.workload]
+    cores = O.n_threads()
+    n = args.cpu_samples or cores                       # one sample per thread per step
+    inp = W.make_all(w, batch=n)
+    for _ in range(min(args.warmup, 1)):                # one warm-up pass is enough for a CPU program
+        oracle_step(w, inp, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(w, inp, n)
+    dt = time.perf_counter() - t0
+    v = n * args.steps / dt
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads.py)",
+        "config": config_of(w, args.batch or w.batch, args.gpus),
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{n} samples of {w.name} per step (sample + log_prob + energy + F_q)"},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_22984_b200 import binding as fv
+    from paper_2606_22984_b200 import build as fvbuild
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not os.path.exists(fv._LIB_PATH):
+        if local == 0:
+            fvbuild.build()
+        if world > 1:
+            dist.barrier()
+
+    w = W.CONFIGS[args.workload]
+    B = args.batch or w.batch
+    inp = W.make_all(w, batch=B, u_seed=W.SEED_U + 1000 * rank)       # each rank: its own sample shard
+    model = fv.create_model(w, inp["weights"], inp["mask_rowptr"], inp["mask_col"], inp["posemb"], B)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    u = d(inp["uniforms"])
+    if w.model == "sk":
+        J = d(inp["J"])
+    else:
+        brp, bcol, bval = d(inp["bond_rowptr"]), d(inp["bond_col"]), d(inp["bond_val"])
+    N = w.n_sites
+    spins = torch.empty((B, N), dtype=torch.int8, device="cuda")
+    logq = torch.empty(B, dtype=torch.float32, device="cuda")
+    logq_tf = torch.empty(B, dtype=torch.float32, device="cuda")
+    E = torch.empty(B, dtype=torch.float32, device="cuda")
+    F = torch.empty(2, dtype=torch.float64, device="cuda")
+    T = 1.0 / w.betas[0]
+
+    def step(evs=None):
+        if evs: evs[0].record()
+        model.sample(u, out=(spins, logq))
+        if evs: evs[1].record()
+        model.log_prob(spins, out=logq_tf)
+        if evs: evs[2].record()
+        if w.model == "sk":
+            fv.energy_dense(spins, J, out=E)
+        else:
+            fv.energy_csr(spins, brp, bcol, bval, w.coupling == "pm1", out=E)
+        fv.free_energy(E, logq_tf, T, out=F)
+        if evs: evs[3].record()
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sync_all()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = fv.launch_count()
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        step(evs[k])
+    sync_all()
+    t1 = time.perf_counter()
+    launches = fv.launch_count() - launches0
+    clocks = sampler.stop(t0, t1) if sampler else None
+    total_ms = evs[0][0].elapsed_time(evs[-1][3])
+    t_sample = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    t_logp = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    t_rest = sum(e[2].elapsed_time(e[3]) for e in evs) / args.steps
+    if world > 1:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = world * B / (ms_per_step * 1e-3)
+
+    # ---- end to end through the public binding with HOST buffers -----------------------------
+    u_host = torch.from_numpy(inp["uniforms"]).pin_memory()
+    spins_host = torch.empty((B, N), dtype=torch.int8).pin_memory()
+    lq_host = torch.empty(B, dtype=torch.float32).pin_memory()
+    E_host = torch.empty(B, dtype=torch.float32).pin_memory()
+    F_host = torch.empty(2, dtype=torch.float64).pin_memory()
+
+    def e2e_step():
+        u.copy_(u_host, non_blocking=True)
+        step()
+        spins_host.copy_(spins, non_blocking=True)
+        lq_host.copy_(logq_tf, non_blocking=True)
+        E_host.copy_(E, non_blocking=True)
+        F_host.copy_(F, non_blocking=True)
+
+    e2e_step()
+    sync_all()
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ea.record()
+    for _ in range(args.steps):
+        e2e_step()
+    eb.record()
+    sync_all()
+    e2e_ms = ea.elapsed_time(eb)
+    if world > 1:
+        tt = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_ms = float(tt.item())
+    e2e_value = world * B / (e2e_ms / args.steps * 1e-3)
+    h2d = u_host.numel() * 4
+    d2h = spins_host.numel() + 4 * B + 4 * B + 16
+    F_val = F_host.clone().numpy()
+
+    if rank == 0:
+        rd, wr = algorithmic_kv_bytes_per_sample(w, inp["mask_rowptr"])
+        peak, peak_src = load_peaks()
+        achieved = (rd + wr) * B / (t_sample * 1e-3) / 1e9
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16 GEMM operands + bf16 KV cache, fp32 accumulate/softmax/LN",
+            "data": "synthetic (seeded couplings, random-init N(0,0.02) weights; workloads.py)",
+            "config": config_of(w, B, world),
+            "phases_ms": {"fv_sample": t_sample, "fv_log_prob": t_logp, "energy+free_energy": t_rest},
+            "us_per_site_step": 1e3 * t_sample / N,
+            "F_q": {"mean": float(F_val[0]), "std": float(F_val[1]), "per_spin": float(F_val[0]) / N},
+            "roofline": {"kernel": "fv_forward_kernel (SAMPLE mode = fv_sample)", "bound": "hbm",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": (rd + wr) * B, "traffic": None},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches), "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            from oracle import oracle as O
+            cores = O.n_threads()
+            n = args.cpu_samples or 2 * cores
+            t0 = time.perf_counter()
+            oracle_step(w, W.make_all(w, batch=n), n)
+            dt = time.perf_counter() - t0
+            out["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                   "sample": f"{n} samples of {w.name} (sample + log_prob + energy + F_q), {dt:.1f} s"}
+        print(json.dumps(out))
+    model.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
