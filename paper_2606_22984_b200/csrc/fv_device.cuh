@@ -1,0 +1,210 @@
+// fv_device.cuh -- device helpers shared by the forward kernels (fv_forward.cu, fv_decode.cu):
+// mma.sync wrapper, packed-weight GEMM over a row tile, LayerNorm row, masked gather attention
+// from global memory, shared-memory geometry.
+#pragma once
+#include "fv_internal.h"
+
+namespace fvdev {
+
+
+constexpr float kLog2e = 1.4426950408889634f;
+
+__device__ __forceinline__ uint32_t lds32(const void* p) { return *reinterpret_cast<const uint32_t*>(p); }
+
+__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint4& a, uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
+        "{%0,%1,%2,%3};\n"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b0), "r"(b1));
+}
+
+// Weights are immutable for the kernel's lifetime: read-only path, keep in L1/L2.
+__device__ __forceinline__ uint4 ldg_w(const uint4* p) { return __ldg(p); }
+
+// KV rows are written by this CTA earlier in the same kernel: coherent (non-.nc) load.
+__device__ __forceinline__ uint4 ld_kv(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];\n" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ float bf_lo(uint32_t x) { return __uint_as_float(x << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// exact GELU, 0.5 x (1 + erf(x / sqrt 2))  (reading A5)
+__device__ __forceinline__ float gelu_erf(float x) { return 0.5f * x * (1.0f + erff(x * 0.70710678118654752f)); }
+
+// Shared-memory geometry (strides chosen so mma fragment accesses are bank-conflict free).
+template <int D, int NT>
+struct Geo {
+    static constexpr int R = 8 * NT;          // rows per tile
+    static constexpr int HS = D + 4;          // fp32 residual stream stride (words)
+    static constexpr int AS = D + 8;          // bf16 activation stride (elements)
+    static constexpr int QS = 3 * D + 4;      // fp32 q|k|v stride (words)
+    static constexpr int FS = 4 * D + 8;      // bf16 FFN hidden stride (elements)
+    static constexpr int KS2 = (D >= 128) ? 2 : 1;   // K-splits of the W2 GEMM
+    static constexpr size_t h_bytes = (size_t)R * HS * 4;
+    static constexpr size_t a_bytes = (size_t)R * AS * 2;
+    static constexpr size_t qkv_bytes = (size_t)R * QS * 4;
+    static constexpr size_t hid_bytes = (size_t)R * FS * 2;
+    static constexpr size_t part_bytes = (size_t)KS2 * R * HS * 4;
+    static constexpr size_t big_bytes = (qkv_bytes > hid_bytes + part_bytes) ? qkv_bytes : hid_bytes + part_bytes;
+    static constexpr size_t split_bytes = (size_t)16 * (D + 2 * (D / 8)) * 4;   // attention split partials
+    static constexpr size_t misc_bytes = (size_t)R * (8 + 4 * 5);            // logq f64, logp, u, tok, b, t
+    static constexpr size_t total = h_bytes + a_bytes + big_bytes + split_bytes + misc_bytes + 64;
+};
+
+// out[row][feat] = sum_k W[feat][k] * act[row][k] for one tile of 8*NT rows.
+// W is pre-packed (fragment order), act is bf16 in shared memory with row stride `as`.
+// Tasks (mt, ks) = (16 output features, one K-split) are dealt round-robin to the warps;
+// epi(mt, ks, acc) receives acc[nt][4]: {(f, r), (f, r+1), (f+8, r), (f+8, r+1)} with
+// f = 16 mt + lane/4 and r = 8 nt + 2 (lane%4).
+template <int KT_TOTAL, int KSPLIT, int NT, int NW, class Epi>
+__device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, const __nv_bfloat16* act, int as,
+                                          int warp, int lane, Epi epi) {
+    constexpr int KT = KT_TOTAL / KSPLIT;
+    constexpr int KU = KT < 8 ? KT : 8;
+    const int g = lane >> 2, c = lane & 3;
+    for (int task = warp; task < MT * KSPLIT; task += NW) {
+        const int mt = task / KSPLIT, ks = task - mt * KSPLIT;
+        float acc[NT][4];
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+        const uint4* w = wp + ((size_t)mt * KT_TOTAL + ks * KT) * 32 + lane;
+        const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+#pragma unroll 1
+        for (int k0 = 0; k0 < KT; k0 += KU) {
+            uint4 a[KU];
+#pragma unroll
+            for (int u = 0; u < KU; ++u) a[u] = ldg_w(w + (k0 + u) * 32);
+#pragma unroll
+            for (int u = 0; u < KU; ++u) {
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const __nv_bfloat16* p = ab + nt * 8 * as + (k0 + u) * 16;
+                    mma_bf16(acc[nt], a[u], lds32(p), lds32(p + 8));
+                }
+            }
+        }
+        epi(mt, ks, acc);
+    }
+}
+
+// LayerNorm of one row held in shared memory (fp32), one warp per row: mean, biased variance,
+// eps inside the sqrt, affine (reading A6).  Writes bf16 to `out`; if `replace` the fp32 row is
+// overwritten with the normalised value (ln2_style 1, Alg. 1 l.5).
+template <int D>
+__device__ __forceinline__ void ln_row(float* hrow, const float* __restrict__ gam, const float* __restrict__ bet,
+                                       float eps, bool replace, __nv_bfloat16* out, int lane) {
+    constexpr int E = D / 32;
+    float x[E];
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < E; ++j) { x[j] = hrow[lane * E + j]; s += x[j]; }
+    const float mean = warp_sum(s) * (1.0f / D);
+    float v = 0.f;
+#pragma unroll
+    for (int j = 0; j < E; ++j) { const float dlt = x[j] - mean; v += dlt * dlt; }
+    const float rstd = rsqrtf(warp_sum(v) * (1.0f / D) + eps);
+#pragma unroll
+    for (int j = 0; j < E; ++j) {
+        const int i = lane * E + j;
+        const float y = (x[j] - mean) * rstd * __ldg(gam + i) + __ldg(bet + i);
+        out[i] = __float2bfloat16_rn(y);
+        if (replace) hrow[i] = y;
+    }
+}
+
+// Masked gather attention for ONE query row against entries [e_begin, e_end) of its CSR mask
+// row (Eq. 3; mask Eq. S1 l.555 generalised to an index list).
+// Lane layout: a KV row is 2D bf16 = K[D] | V[D]; LPR = D/8 lanes cover K (16 B each) and the
+// same lanes fetch the matching 16 B of V, so a warp handles RPI = 32/LPR rows per iteration.
+// A head spans LPH = DH/8 adjacent lanes; its score is completed by shfl.xor over them.
+// Online softmax in base 2 (q is pre-scaled by log2(e)/sqrt(d_h)); state (m, l, acc[8]) is per
+// lane and merged across the RPI row groups at the end, so every lane returns the result.
+template <int D, int DH>
+__device__ __forceinline__ void attend_range(const float* qrow, const __nv_bfloat16* kv_sl, const int32_t* __restrict__ cols,
+                                             int e_begin, int e_end, int lane, float& m_out, float& l_out,
+                                             float (&acc)[8]) {
+    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8, U = 4;
+    const int rg = lane / LPR, sub = lane % LPR;
+    const float qs = kLog2e * rsqrtf((float)DH);
+    float q[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) q[j] = qrow[sub * 8 + j] * qs;
+    float m = -1e30f, l = 0.f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+    const char* base = reinterpret_cast<const char*>(kv_sl) + sub * 16;
+    for (int e0 = e_begin; e0 < e_end; e0 += RPI * U) {
+        uint4 kk[U], vv[U];
+        bool ok[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int e = e0 + u * RPI + rg;
+            ok[u] = e < e_end;
+            const int pos = __ldg(cols + (ok[u] ? e : e_begin));
+            const char* p = base + (size_t)pos * (4 * D);
+            kk[u] = ld_kv(p);
+            vv[u] = ld_kv(p + 2 * D);
+        }
+        float s[U];
+        float mx = m;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
+            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
+            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
+            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
+#pragma unroll
+            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+            s[u] = ok[u] ? d : -INFINITY;
+            mx = fmaxf(mx, s[u]);
+        }
+        const float corr = exp2f(m - mx);
+        m = mx;
+        l *= corr;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] *= corr;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const float p = exp2f(s[u] - mx);
+            l += p;
+            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
+            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
+            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
+            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
+        }
+    }
+#pragma unroll
+    for (int o = LPR; o < 32; o <<= 1) {       // merge the RPI row groups
+        const float m2 = __shfl_xor_sync(0xffffffffu, m, o);
+        const float l2 = __shfl_xor_sync(0xffffffffu, l, o);
+        const float mx = fmaxf(m, m2);
+        const float c1 = exp2f(m - mx), c2 = exp2f(m2 - mx);
+        l = l * c1 + l2 * c2;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float a2 = __shfl_xor_sync(0xffffffffu, acc[j], o);
+            acc[j] = acc[j] * c1 + a2 * c2;
+        }
+        m = mx;
+    }
+    m_out = m;
+    l_out = l;
+}
+
+
+}  // namespace fvdev
