@@ -1,7 +1,9 @@
 // fv_api.cu -- the extern "C" boundary of libflashvan.so (see include/flashvan.h).
 // Host orchestration only: argument validation, one-off weight packing, launch geometry.
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -168,6 +170,28 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     const size_t o_pos = A.put(posemb, sizeof(float) * (size_t)N * (d - cfg->d_token));
     const size_t o_rp = A.put(mask_rowptr, sizeof(int32_t) * (N + 1));
     const size_t o_col = A.put(mask_col, sizeof(int32_t) * (size_t)mask_rowptr[N]);
+    // KV ring copy plan (fv_decode.cu): chunks of CH rows of A(t) \ {t}, runs of consecutive positions
+    const int CH = fv_ring_ch(d);
+    std::vector<int32_t> chunk_ptr(N + 1, 0), chunk_run_ptr(1, 0);
+    std::vector<int2> runs;
+    for (int t = 0; t < N; ++t) {
+        const int e0 = mask_rowptr[t], nn = mask_rowptr[t + 1] - 1 - e0;
+        for (int c0 = 0; c0 < nn; c0 += CH) {
+            const int rows = std::min(CH, nn - c0);
+            for (int i = 0; i < rows;) {
+                int j = i + 1;
+                while (j < rows && mask_col[e0 + c0 + j] == mask_col[e0 + c0 + j - 1] + 1) ++j;
+                runs.push_back(make_int2(mask_col[e0 + c0 + i], (i << 16) | (j - i)));
+                i = j;
+            }
+            chunk_run_ptr.push_back((int32_t)runs.size());
+        }
+        chunk_ptr[t + 1] = (int32_t)chunk_run_ptr.size() - 1;
+    }
+    if (runs.empty()) runs.push_back(make_int2(0, 0));
+    const size_t o_cp = A.put(chunk_ptr.data(), sizeof(int32_t) * chunk_ptr.size());
+    const size_t o_crp = A.put(chunk_run_ptr.data(), sizeof(int32_t) * chunk_run_ptr.size());
+    const size_t o_runs = A.put(runs.data(), sizeof(int2) * runs.size());
 
     m->arena_bytes = A.host.size();
     e = cudaMalloc(&m->arena, m->arena_bytes);
@@ -191,6 +215,9 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.head_bd = bd;
     D.mask_rowptr = (const int32_t*)(base + o_rp);
     D.mask_col = (const int32_t*)(base + o_col);
+    D.chunk_ptr = (const int32_t*)(base + o_cp);
+    D.chunk_run_ptr = (const int32_t*)(base + o_crp);
+    D.runs = (const int2*)(base + o_runs);
     D.kv = (__nv_bfloat16*)kv;
     for (int l = 0; l < NL; ++l) {
         const Off& o = off[l];
@@ -242,8 +269,8 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
     int nt, grid;
     sample_geometry(B, m->n_sms, &a.rows_per_group, &nt, &a.n_groups, &grid);
     a.uniforms = uniforms; a.spins_out = spins; a.logq = logq; a.cond_p = cond_p;
-    cudaError_t e = fv_launch_forward(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, grid,
-                                      (cudaStream_t)stream);
+    cudaError_t e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, grid,
+                                     (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "fv_sample launch");
     g_launches++;
     return FV_OK;

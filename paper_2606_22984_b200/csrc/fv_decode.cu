@@ -1,0 +1,551 @@
+// fv_decode.cu -- the persistent KV-cached sampler of fv_sample (Alg. 2) for sm_100a.
+//
+// A CTA owns a group of S <= 8*NT samples for all N steps (samples are independent, l.125, so
+// CTAs never communicate).  Per step t and layer: LN1 -> QKV -> KV append -> masked attention
+// over the rows A(t) of the CSR mask -> (W_O) -> LN2 -> FFN -> residual; then the sigmoid head,
+// the Bernoulli draw from the caller's uniform and the log q update.
+//
+// What is new against fv_forward.cu (still used by fv_log_prob): the KV gather is decoupled from
+// the compute warps.  The mask is static, so every KV row a step will need -- except the row the
+// step itself appends -- is known long before; one PRODUCER warp walks (t, layer, sample) in the
+// consumers' order and streams the rows named by the mask from the bf16 KV pool into a shared
+// memory ring with cp.async.bulk (TMA 1-D bulk copies, runs of consecutive positions merged into
+// one copy), completing on mbarriers.  The 16 COMPUTE warps read K/V from shared memory, so HBM
+// keeps streaming during the GEMM phases instead of idling (profiles/r01: attention phase 51 %
+// of the step, HBM idle in the other 49 %).  Row t itself is taken from the registers/shared
+// memory of the step that produced it (rounded to bf16 exactly as the pool stores it).
+#include <cstdio>
+#include "fv_device.cuh"
+
+// Tuning knobs (compile time; the defaults are the measured best).
+#ifndef FV_DEC_ORDER
+#define FV_DEC_ORDER 1      // ring order: 0 = sample-major, 1 = chunk-major
+#endif
+#ifndef FV_DEC_MAXL
+#define FV_DEC_MAXL 8       // 128-bit weight loads in flight per lane in the GEMM phases
+#endif
+#ifndef FV_DEC_WNA
+#define FV_DEC_WNA 0        // 1: weight loads do not allocate in L1
+#endif
+#ifndef FV_DEC_SLOTS
+#define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
+#endif
+
+namespace {
+using namespace fvdev;
+
+constexpr int NWC = 16;                       // compute warps
+constexpr int NTHREADS = NWC * 32 + 32;       // + 1 producer warp
+constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
+
+template <int D, int NT>
+struct DecGeo {
+    using G = Geo<D, NT>;
+    static constexpr int CH = fv_ring_ch(D);              // KV rows per ring chunk (host plan agrees)
+    static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
+    static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
+    static constexpr size_t fixed = (G::total + 127) / 128 * 128;
+    static constexpr int TAB_C = 128, TAB_R = 320;        // per-step copy plan staged in smem
+    static constexpr size_t bar_bytes = 1024 + TAB_C * 4 + TAB_R * 8;   // 2 x 60 mbarriers, counter, plan
+    static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
+    static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
+    static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
+    static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
+    static_assert(NSLOT >= 2, "KV ring needs at least two chunks");
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int who = 0, uint32_t tag = 0) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+#ifdef FV_DEC_WATCHDOG
+    long long spins = 0;
+#endif
+    do {
+#ifdef FV_DEC_WATCHDOG
+        if (++spins > 4000000) {
+            printf("WATCHDOG who=%d cta=%d warp=%d lane=%d tag=%u parity=%u\n", who, blockIdx.x, threadIdx.x >> 5,
+                   threadIdx.x & 31, tag, parity);
+            return;
+        }
+#endif
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!done);
+}
+// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWC * 32) : "memory"); }
+__device__ __forceinline__ int ld_acquire_s32(const int* p) {
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];\n" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_s32(int* p, int v) {
+    asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ float bf16_round(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
+
+// Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
+// PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
+// with 128-bit shared loads and the matching 16 B of V; RPI = 32/LPR rows per iteration.
+template <int D, int DH, int CH>
+__device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
+                                             float& m, float& l, float (&acc)[8]) {
+    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
+    constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
+    const unsigned char* base = chunk + sub * 16;
+    for (int i0 = 0; i0 < rows; i0 += RPI * U) {
+        uint4 kk[U], vv[U];
+        bool ok[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int row = i0 + u * RPI + rg;
+            ok[u] = row < rows;
+            const unsigned char* p = base + (size_t)(ok[u] ? row : 0) * (4 * D);
+            kk[u] = *reinterpret_cast<const uint4*>(p);
+            vv[u] = *reinterpret_cast<const uint4*>(p + 2 * D);
+        }
+        float s[U];
+        float mx = m;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
+            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
+            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
+            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
+#pragma unroll
+            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+            s[u] = ok[u] ? d : -INFINITY;
+            mx = fmaxf(mx, s[u]);
+        }
+        const float corr = exp2f(m - mx);
+        m = mx;
+        l *= corr;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] *= corr;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const float p = exp2f(s[u] - mx);
+            l += p;
+            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
+            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
+            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
+            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
+        }
+    }
+}
+
+template <int D, int DH, int NT>
+__global__ void __launch_bounds__(NTHREADS, 1)
+fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
+    using G = Geo<D, NT>;
+    using DG = DecGeo<D, NT>;
+    constexpr int R = G::R, HS = G::HS, AS = G::AS, QS = G::QS, FS = G::FS, KS2 = G::KS2;
+    constexpr int NSPLIT = (NWC / R) > 1 ? (NWC / R) : 1;    // warps cooperating on one query row
+    constexpr int LPR = D / 8, LPH = DH / 8;
+    constexpr int SPS = D + 2 * LPR;                          // floats per split-partial slot
+    constexpr int GR = NWC / NSPLIT;                          // samples attended at the same time
+    constexpr int CH = DG::CH, NSLOT = DG::NSLOT, NSLOT_MAX = DG::NSLOT;
+    static_assert(R * NSPLIT <= 16 || NSPLIT == 1, "split slots");
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    float* sh_h = reinterpret_cast<float*>(smem);
+    __nv_bfloat16* sh_a = reinterpret_cast<__nv_bfloat16*>(smem + G::h_bytes);
+    unsigned char* big = smem + G::h_bytes + G::a_bytes;
+    float* sh_qkv = reinterpret_cast<float*>(big);
+    __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
+    float* sh_part = reinterpret_cast<float*>(big + G::hid_bytes);
+    float* sh_split = reinterpret_cast<float*>(big + G::big_bytes);
+    double* sh_logq = reinterpret_cast<double*>(big + G::big_bytes + G::split_bytes);
+    float* sh_logp = reinterpret_cast<float*>(sh_logq + R);
+    float* sh_u = sh_logp + R;
+    int* sh_tok = reinterpret_cast<int*>(sh_u + R);
+    uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + DG::fixed);
+    uint64_t* bar_empty = bar_full + NSLOT_MAX;
+    int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
+    int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
+    int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
+    int2* tab_r = reinterpret_cast<int2*>(tab_c + DG::TAB_C);
+    unsigned char* ring = smem + DG::fixed + DG::bar_bytes;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int N = m.n_sites, NL = m.n_layers;
+
+    if (tid == 0) {
+        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
+        *sh_app = 0;
+        *sh_issued = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+
+    // =============================== PRODUCER WARP ===============================
+    // Lanes work on VW consecutive chunks of the ring at once (one chunk per lane: wait for the
+    // slot, arm the mbarrier, one bulk copy per run).  VW <= NSLOT, so a lane only ever waits
+    // on a chunk issued in an earlier round -- no circular wait with the consumers.
+    if (warp == NWC) {
+        constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
+        uint32_t seq = 0;
+        int it = 0;
+        for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
+            const int b_first = unit * a.rows_per_group;
+            const int n_own = min(a.rows_per_group, a.B - b_first);
+            for (int t = 1; t < N; ++t) {
+                const int cp0 = __ldg(m.chunk_ptr + t);
+                const int nch = __ldg(m.chunk_ptr + t + 1) - cp0;
+                if (nch == 0) continue;
+                const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
+                // stage this step's copy plan in shared memory (it is reused n_l * n_own times)
+                const int rp0 = __ldg(m.chunk_run_ptr + cp0);
+                const int nruns = __ldg(m.chunk_run_ptr + cp0 + nch) - rp0;
+                const int32_t* cptr;
+                const int2* rptr;
+                __syncwarp();
+                if (nch + 1 <= DG::TAB_C && nruns <= DG::TAB_R) {
+                    for (int i = lane; i <= nch; i += 32) tab_c[i] = __ldg(m.chunk_run_ptr + cp0 + i) - rp0;
+                    for (int i = lane; i < nruns; i += 32) tab_r[i] = __ldg(m.runs + rp0 + i);
+                    __syncwarp();
+                    cptr = tab_c; rptr = tab_r;
+                } else {
+                    cptr = m.chunk_run_ptr + cp0; rptr = m.runs;
+                }
+                const int total = n_own * nch;
+                for (int l = 0; l < NL; ++l) {
+                    // rows < t of layer l are complete once step t-1 has appended at layer l
+                    const int need = (it * N + (t - 1)) * NL + l + 1;
+                    while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
+                    const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
+                        m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
+                    for (int i0 = 0; i0 < total; i0 += VW) {
+                        const int i = i0 + lane;
+                        if (lane < VW && i < total) {
+                            int r, c;
+                            if (FV_DEC_ORDER) {
+                                // chunk-major inside a round of GR samples (= the samples the compute
+                                // warps work on at the same time), rounds in order: every warp then
+                                // consumes its chunks in ring order
+                                const int k = i / (GR * nch), rem = i - k * GR * nch;
+                                const int nk = min(GR, n_own - k * GR);
+                                c = rem / nk;
+                                r = k * GR + (rem - c * nk);
+                            } else { r = i / nch; c = i - r * nch; }                  // sample-major
+                            const uint32_t sq = seq + (uint32_t)i;
+                            const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                            mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
+                            const int rows = min(CH, nn - c * CH);
+                            mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * DG::ROW_BYTES);
+                            const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
+                            unsigned char* dst = ring + (size_t)slot * DG::CHUNK_BYTES;
+                            const int j1 = cptr[c + 1];
+                            for (int j = cptr[c]; j < j1; ++j) {
+                                const int2 run = rptr[j];
+                                bulk_g2s(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
+                                         (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot);
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, total)));
+                    }
+                    seq += (uint32_t)total;
+                }
+            }
+        }
+        return;
+    }
+
+    // =============================== COMPUTE WARPS ===============================
+    const int g = lane >> 2, c4 = lane & 3;
+    const int rg = lane / LPR, sub = lane % LPR;
+    uint32_t seq_base = 0;
+    int it = 0;
+    for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
+        const int b_first = unit * a.rows_per_group;
+        const int n_own = min(a.rows_per_group, a.B - b_first);
+        if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
+        for (int t = 0; t < N; ++t) {
+            const int me0 = __ldg(m.mask_rowptr + t);
+            const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
+            const int nch = (nn + CH - 1) / CH;
+            if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
+            cbar();
+            // ---- concatenated positional embedding (Eq. 15, l.287-292) -------------------
+            for (int i = tid; i < R * D; i += NWC * 32) {
+                const int r = i / D, f = i - r * D;
+                const int dt = m.d_token;
+                sh_h[r * HS + f] = f < dt ? __ldg(m.tok_emb + sh_tok[r] * dt + f)
+                                          : __ldg(m.posemb + (size_t)t * (D - dt) + (f - dt));
+            }
+            cbar();
+            for (int l = 0; l < NL; ++l) {
+                const FvLayerDev& L = m.layer[l];
+                // ---- LN1 (Alg. 2 l.12) -> bf16 activations ----------------------------------
+                for (int r = warp; r < R; r += NWC)
+                    ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+                cbar();
+                // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13) ---------------------------------
+                gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane,
+                    [&](int mt, int, float (&acc)[NT][4]) {
+                        const int f = mt * 16 + g;
+                        const float b0 = __ldg(L.bqkv + f), b1 = __ldg(L.bqkv + f + 8);
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) {
+                            float* o = sh_qkv + (nt * 8 + 2 * c4) * QS + f;
+                            o[0] = acc[nt][0] + b0; o[QS] = acc[nt][1] + b0;
+                            o[8] = acc[nt][2] + b1; o[QS + 8] = acc[nt][3] + b1;
+                        }
+                    });
+                cbar();
+                // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) -------
+                for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
+                    const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
+                    if (r >= n_own) continue;
+                    const float* s = sh_qkv + r * QS + D + ch * 8;
+                    uint4 v;
+                    v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
+                    v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
+                    __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
+                    *reinterpret_cast<uint4*>(dst) = v;
+                }
+                // the producer reads these rows through the async proxy (cp.async.bulk)
+                asm volatile("fence.proxy.async.global;\n" ::: "memory");
+                cbar();
+                if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
+                // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
+                for (int task = warp; task < R * NSPLIT; task += NWC) {
+                    const int r = task / NSPLIT, sp = task - r * NSPLIT;
+                    if (r >= n_own) continue;
+                    const float qs = kLog2e * rsqrtf((float)DH);
+                    const float* qrow = sh_qkv + r * QS;
+                    float q[8], acc[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) q[j] = qrow[sub * 8 + j] * qs;
+                    float mm = -1e30f, ll = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+                    if (sp == 0) {                       // row t itself, as the pool stores it (bf16)
+                        float d = 0.f;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) d += q[j] * bf16_round(qrow[D + sub * 8 + j]);
+#pragma unroll
+                        for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+                        if (rg == 0) {
+                            mm = d; ll = 1.f;
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) acc[j] = bf16_round(qrow[2 * D + sub * 8 + j]);
+                        }
+                    }
+                    for (int c = sp; c < nch; c += NSPLIT) {
+                        const int kr = r / GR, nk = min(GR, n_own - kr * GR);
+                        const uint32_t sq = seq_base + (uint32_t)(FV_DEC_ORDER ? kr * GR * nch + c * nk + (r - kr * GR)
+                                                                               : r * nch + c);
+                        const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                        // A parity wait can only tell a phase from its predecessor: make sure the
+                        // producer has armed THIS round of the slot before waiting on it (another
+                        // warp may still own the slot's previous round).
+                        while ((int)((uint32_t)ld_acquire_s32(sh_issued) - sq) <= 0) __nanosleep(20);
+                        mbar_wait(bar_full + slot, par, 2, sq);
+                        attend_chunk<D, DH, CH>(ring + (size_t)slot * DG::CHUNK_BYTES, min(CH, nn - c * CH), q, rg, sub,
+                                                mm, ll, acc);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar_empty + slot);
+                    }
+#pragma unroll
+                    for (int o = LPR; o < 32; o <<= 1) {       // merge the RPI row groups
+                        const float m2 = __shfl_xor_sync(0xffffffffu, mm, o);
+                        const float l2 = __shfl_xor_sync(0xffffffffu, ll, o);
+                        const float mx = fmaxf(mm, m2);
+                        const float c1 = exp2f(mm - mx), c2 = exp2f(m2 - mx);
+                        ll = ll * c1 + l2 * c2;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const float a2 = __shfl_xor_sync(0xffffffffu, acc[j], o);
+                            acc[j] = acc[j] * c1 + a2 * c2;
+                        }
+                        mm = mx;
+                    }
+                    if (lane < LPR) {
+                        if (NSPLIT > 1) {
+                            float* ps = sh_split + task * SPS;
+                            ps[lane] = mm; ps[LPR + lane] = ll;
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) ps[2 * LPR + lane * 8 + j] = acc[j];
+                        } else {
+                            const float inv = 1.0f / ll;
+                            if (m.has_wo) {
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) sh_a[r * AS + lane * 8 + j] = __float2bfloat16_rn(acc[j] * inv);
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < 8; ++j) sh_h[r * HS + lane * 8 + j] += acc[j] * inv;
+                            }
+                        }
+                    }
+                }
+                seq_base += (uint32_t)(n_own * nch);
+                cbar();
+                if (NSPLIT > 1) {                       // combine the split partials, fixed order
+                    for (int i = tid; i < R * D; i += NWC * 32) {
+                        const int r = i / D, f = i - r * D;
+                        if (r >= n_own) continue;
+                        const float* ps = sh_split + r * NSPLIT * SPS;
+                        float mx = -1e30f;
+#pragma unroll
+                        for (int s = 0; s < NSPLIT; ++s) mx = fmaxf(mx, ps[s * SPS + f / 8]);
+                        float num = 0.f, den = 0.f;
+#pragma unroll
+                        for (int s = 0; s < NSPLIT; ++s) {
+                            const float w = exp2f(ps[s * SPS + f / 8] - mx);
+                            den += w * ps[s * SPS + LPR + f / 8];
+                            num += w * ps[s * SPS + 2 * LPR + f];
+                        }
+                        const float u = num / den;
+                        if (m.has_wo) sh_a[r * AS + f] = __float2bfloat16_rn(u);
+                        else sh_h[r * HS + f] += u;
+                    }
+                    cbar();
+                }
+                // ---- optional output projection (bypassed in the paper, l.107) --------------
+                if (m.has_wo) {
+                    gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane,
+                        [&](int mt, int, float (&acc)[NT][4]) {
+                            const int f = mt * 16 + g;
+                            const float b0 = __ldg(L.bo + f), b1 = __ldg(L.bo + f + 8);
+#pragma unroll
+                            for (int nt = 0; nt < NT; ++nt) {
+                                float* o = sh_h + (nt * 8 + 2 * c4) * HS + f;
+                                o[0] += acc[nt][0] + b0; o[HS] += acc[nt][1] + b0;
+                                o[8] += acc[nt][2] + b1; o[HS + 8] += acc[nt][3] + b1;
+                            }
+                        });
+                    cbar();
+                }
+                // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
+                for (int r = warp; r < R; r += NWC)
+                    ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                cbar();
+                // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
+                gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane,
+                    [&](int mt, int, float (&acc)[NT][4]) {
+                        const int f = mt * 16 + g;
+                        const float b0 = __ldg(L.b1 + f), b1 = __ldg(L.b1 + f + 8);
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) {
+                            __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS + f;
+                            o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
+                            o[FS] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
+                            o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
+                            o[FS + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
+                        }
+                    });
+                cbar();
+                // ---- FFN down-projection, K split KS2 ways into partial buffers -------------
+                gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane,
+                    [&](int mt, int ks, float (&acc)[NT][4]) {
+                        const int f = mt * 16 + g;
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) {
+                            float* o = sh_part + ((size_t)ks * R + nt * 8 + 2 * c4) * HS + f;
+                            o[0] = acc[nt][0]; o[HS] = acc[nt][1];
+                            o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
+                        }
+                    });
+                cbar();
+                // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
+                for (int i = tid; i < R * D; i += NWC * 32) {
+                    const int r = i / D, f = i - r * D;
+                    float v = __ldg(L.b2 + f);
+#pragma unroll
+                    for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                    sh_h[r * HS + f] += v;
+                }
+                cbar();
+            }
+            // ---- output head: p(+1) = softmax(z)[1] = sigmoid(z1 - z0) (Alg. 2 l.20-22) -----
+            for (int r = warp; r < R; r += NWC) {
+                if (r >= n_own) continue;
+                const int b = b_first + r;
+                float d = 0.f;
+#pragma unroll
+                for (int j = 0; j < D / 32; ++j) d += sh_h[r * HS + lane * (D / 32) + j] * __ldg(m.head_wd + lane * (D / 32) + j);
+                d = warp_sum(d) + m.head_bd;
+                if (lane == 0) {
+                    const float p = 1.0f / (1.0f + expf(-d));
+                    const int up = sh_u[r] < p;                            // reading A10 (l.23)
+                    a.spins_out[(size_t)b * N + t] = up ? 1 : -1;           // sigma = 2 s - 1 (l.25)
+                    sh_tok[r] = up;
+                    const float x = up ? -d : d;                           // log p(s) = -softplus(x)
+                    sh_logp[r] = -(fmaxf(x, 0.f) + log1pf(expf(-fabsf(x))));
+                    if (a.cond_p) a.cond_p[(size_t)b * N + t] = p;
+                }
+            }
+            cbar();
+            // ---- log q accumulation in fp64, fixed order (Alg. 1 l.9) --------------------------
+            if (tid < n_own) {
+                sh_logq[tid] += (double)sh_logp[tid];
+                if (t == N - 1) a.logq[b_first + tid] = (float)sh_logq[tid];
+            }
+        }
+        cbar();
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------ dispatch
+template <int D, int DH, int NT>
+static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int grid, cudaStream_t s) {
+    auto kern = fv_decode_kernel<D, DH, NT>;
+    using DG = DecGeo<D, NT>;
+    const size_t smem = DG::total;
+    static bool attr_set = false;                 // per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DG::total);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    kern<<<grid, NTHREADS, smem, s>>>(m, a);
+    return cudaGetLastError();
+}
+
+template <int D, int DH>
+static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArgs& a, int grid, cudaStream_t s) {
+    switch (nt) {
+        case 1: return launch_dec<D, DH, 1>(m, a, grid, s);
+        case 2: return launch_dec<D, DH, 2>(m, a, grid, s);
+        case 4: return launch_dec<D, DH, 4>(m, a, grid, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt, const FvForwardArgs& a,
+                             int grid, cudaStream_t s) {
+    const int key = d_model * 1000 + d_head;
+    switch (key) {
+#ifndef FV_DEC_ONLY_128_16
+        case 32016: return launch_dec_nt<32, 16>(m, nt, a, grid, s);
+        case 64016: return launch_dec_nt<64, 16>(m, nt, a, grid, s);
+        case 64032: return launch_dec_nt<64, 32>(m, nt, a, grid, s);
+        case 128032: return launch_dec_nt<128, 32>(m, nt, a, grid, s);
+        case 256064: return launch_dec_nt<256, 64>(m, nt, a, grid, s);
+#endif
+        case 128016: return launch_dec_nt<128, 16>(m, nt, a, grid, s);
+        default: return cudaErrorInvalidValue;
+    }
+}

@@ -21,6 +21,13 @@ __device__ __forceinline__ void mma_bf16(float (&c)[4], const uint4& a, uint32_t
 
 // Weights are immutable for the kernel's lifetime: read-only path, keep in L1/L2.
 __device__ __forceinline__ uint4 ldg_w(const uint4* p) { return __ldg(p); }
+// Streaming variant: no L1 allocation (nothing is reused by this SM within a phase).
+__device__ __forceinline__ uint4 ldg_w_na(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
 
 // KV rows are written by this CTA earlier in the same kernel: coherent (non-.nc) load.
 __device__ __forceinline__ uint4 ld_kv(const void* p) {
@@ -71,34 +78,57 @@ struct Geo {
 // Tasks (mt, ks) = (16 output features, one K-split) are dealt round-robin to the warps;
 // epi(mt, ks, acc) receives acc[nt][4]: {(f, r), (f, r+1), (f+8, r), (f+8, r+1)} with
 // f = 16 mt + lane/4 and r = 8 nt + 2 (lane%4).
-template <int KT_TOTAL, int KSPLIT, int NT, int NW, class Epi>
+// The weight stream comes from L2 (latency ~1 us under load) and nothing is reused, so the
+// loads of up to TPB tasks (MAXL x 128-bit per lane) are issued before the first MMA: one L2
+// round trip per GEMM phase instead of one per task.
+template <int KT_TOTAL, int KSPLIT, int NT, int NW, int MAXL = 16, bool NA = false, class Epi>
 __device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, const __nv_bfloat16* act, int as,
                                           int warp, int lane, Epi epi) {
     constexpr int KT = KT_TOTAL / KSPLIT;
-    constexpr int KU = KT < 8 ? KT : 8;
+    constexpr int KU = KT < MAXL ? KT : MAXL;
+    constexpr int TPB = (MAXL / KU) < 4 ? (MAXL / KU) : 4;
     const int g = lane >> 2, c = lane & 3;
-    for (int task = warp; task < MT * KSPLIT; task += NW) {
-        const int mt = task / KSPLIT, ks = task - mt * KSPLIT;
-        float acc[NT][4];
+    const int total = MT * KSPLIT;
+    for (int task0 = warp; task0 < total; task0 += NW * TPB) {
+        uint4 a[TPB][KU];
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
-        const uint4* w = wp + ((size_t)mt * KT_TOTAL + ks * KT) * 32 + lane;
-        const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
-#pragma unroll 1
-        for (int k0 = 0; k0 < KT; k0 += KU) {
-            uint4 a[KU];
+        for (int tb = 0; tb < TPB; ++tb) {
+            const int task = task0 + tb * NW;
+            if (task < total) {
+                const int mt = task / KSPLIT, ks = task - mt * KSPLIT;
+                const uint4* w = wp + ((size_t)mt * KT_TOTAL + ks * KT) * 32 + lane;
 #pragma unroll
-            for (int u = 0; u < KU; ++u) a[u] = ldg_w(w + (k0 + u) * 32);
-#pragma unroll
-            for (int u = 0; u < KU; ++u) {
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    const __nv_bfloat16* p = ab + nt * 8 * as + (k0 + u) * 16;
-                    mma_bf16(acc[nt], a[u], lds32(p), lds32(p + 8));
-                }
+                for (int u = 0; u < KU; ++u) a[tb][u] = NA ? ldg_w_na(w + u * 32) : ldg_w(w + u * 32);
             }
         }
-        epi(mt, ks, acc);
+#pragma unroll
+        for (int tb = 0; tb < TPB; ++tb) {
+            const int task = task0 + tb * NW;
+            if (task < total) {
+                const int mt = task / KSPLIT, ks = task - mt * KSPLIT;
+                float acc[NT][4];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+                const uint4* w = wp + ((size_t)mt * KT_TOTAL + ks * KT) * 32 + lane;
+                const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+#pragma unroll 1
+                for (int k0 = 0; k0 < KT; k0 += KU) {
+                    if (k0 > 0) {
+#pragma unroll
+                        for (int u = 0; u < KU; ++u) a[tb][u] = NA ? ldg_w_na(w + (k0 + u) * 32) : ldg_w(w + (k0 + u) * 32);
+                    }
+#pragma unroll
+                    for (int u = 0; u < KU; ++u) {
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) {
+                            const __nv_bfloat16* p = ab + nt * 8 * as + (k0 + u) * 16;
+                            mma_bf16(acc[nt], a[tb][u], lds32(p), lds32(p + 8));
+                        }
+                    }
+                }
+                epi(mt, ks, acc);
+            }
+        }
     }
 }
 

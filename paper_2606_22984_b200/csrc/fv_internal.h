@@ -6,6 +6,12 @@
 
 #define FV_MAX_LAYERS 16
 
+// KV rows per ring chunk of the decode kernel (host plan and device kernel must agree).
+#ifndef FV_DEC_CH128
+#define FV_DEC_CH128 16
+#endif
+constexpr int fv_ring_ch(int d_model) { return d_model >= 256 ? 8 : (d_model >= 128 ? FV_DEC_CH128 : 16); }
+
 // Per-layer device pointers.  GEMM weights are bf16, pre-packed at fv_create_model time into
 // mma.m16n8k16 A-fragment order: tile (mt, kt) of W[out,in] is 32 lanes x 16 B, contiguous,
 // so one warp-wide 128-bit load fetches a whole 16x16 tile (see pack_mma_a in fv_api.cu).
@@ -28,6 +34,12 @@ struct FvModelDev {
     float head_bd;          //      = head_b[1] - head_b[0]
     const int32_t* mask_rowptr;
     const int32_t* mask_col;
+    // KV ring copy plan of fv_decode.cu (derived from the mask at fv_create_model): row t minus its own
+    // entry is cut into chunks of fv_ring_ch(d) rows; each chunk is a list of runs of consecutive
+    // positions, one cp.async.bulk per run.  run.x = first position, run.y = (row in chunk << 16) | length.
+    const int32_t* chunk_ptr;      // [N+1]  chunks before step t
+    const int32_t* chunk_run_ptr;  // [n_chunks+1]
+    const int2* runs;
     __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16)
     FvLayerDev layer[FV_MAX_LAYERS];
 };
@@ -51,6 +63,8 @@ struct FvForwardArgs {
 cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int nt,
                               const FvForwardArgs& a, int grid, cudaStream_t s);
 size_t fv_forward_smem_bytes(int d_model, int nt);
+cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt,
+                             const FvForwardArgs& a, int grid, cudaStream_t s);
 cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_t* rowptr,
                                  const int32_t* col, const float* val, int integer, float* E,
                                  cudaStream_t s);

@@ -156,3 +156,37 @@ def test_batch_edges_and_errors():
     a = model.sample(u, want_cond_p=True)
     b = model.sample(u, want_cond_p=True)
     assert all(torch.equal(x, y) for x, y in zip(a, b))
+
+
+# ------------------------------------------- full BASELINE sizes, bench.py's launch configuration
+@pytest.mark.parametrize("name,n_check", [("cfg2", 16), ("cfg3", 6), ("cfg4", 6), ("cfg5", 3)])
+def test_full_size_sampled_rows(name, n_check):
+    """fv_sample and fv_log_prob at the full batch and length of the BASELINE config (the launch
+    geometry bench.py times: samples per CTA, ring smaller than a layer-step, several rounds per
+    CTA), checked on a few samples the oracle can afford: first, last and evenly spread ones."""
+    w = W.CONFIGS[name]
+    B = w.batch
+    model, weights, posemb, rp, col = build(w, B)
+    u = W.make_uniforms(w, B)
+    spins_g, lq_g, cp_g = model.sample(dev(u), want_cond_p=True)
+    lq_tf, cp_tf = model.log_prob(spins_g, want_cond_p=True)
+    torch.cuda.synchronize()
+    idx = np.unique(np.linspace(0, B - 1, n_check).astype(np.int64))
+    s = spins_g[idx].cpu().numpy()
+    assert set(np.unique(spins_g.cpu().numpy())) <= {-1, 1}
+    lq_o, cp_o = O.log_prob(w, weights, posemb, rp, col, s)
+    cp_s = cp_g[idx].cpu().numpy().astype(np.float64)
+    assert np.abs(cp_s - cp_o).max() <= TOL_P, np.abs(cp_s - cp_o).max()
+    assert np.abs(cp_tf[idx].cpu().numpy().astype(np.float64) - cp_o).max() <= TOL_P
+    uu = u[idx].astype(np.float64)
+    mism = s != np.where(uu < cp_o, 1, -1)
+    tie = np.abs(uu - cp_o) < TOL_P
+    assert not (mism & ~tie).any()
+    picked = np.where(s > 0, cp_o, 1 - cp_o)
+    bound = TOL_P * (1.0 / picked).sum(1) + 1e-4 * np.abs(lq_o)
+    assert (np.abs(lq_g[idx].cpu().numpy().astype(np.float64) - lq_o) <= bound).all()
+    assert (np.abs(lq_tf[idx].cpu().numpy().astype(np.float64) - lq_o) <= bound).all()
+    # every sample: finite, and the two GPU passes agree with each other (chain rule)
+    assert torch.isfinite(lq_g).all() and torch.isfinite(lq_tf).all()
+    assert (lq_g - lq_tf).abs().max().item() <= 2e-4 * max(1.0, lq_g.abs().max().item())
+    model.close()
