@@ -27,6 +27,9 @@
 #ifndef FV_DEC_WNA
 #define FV_DEC_WNA 0        // 1: weight loads do not allocate in L1
 #endif
+#ifndef FV_DEC_WRING
+#define FV_DEC_WRING 1      // 1: GEMM weights stream through the shared-memory ring (TMA), 0: LDG from L2
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -51,6 +54,14 @@ struct DecGeo {
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
     static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
     static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
+    // GEMM weights stream through the same ring (D <= 128): a chunk is CHUNK_BYTES of the packed
+    // image = TPCH 16x16 tiles = whole m-tiles (K = D) or one K-part of an m-tile (K = 4D).
+    static constexpr bool WRING = FV_DEC_WRING && D <= 128;
+    static constexpr int TPCH = CHUNK_BYTES / 512;
+    static constexpr int NQ = (3 * D / 16) * (D / 16) / TPCH;     // W_qkv chunks
+    static constexpr int NO = (D / 16) * (D / 16) / TPCH;         // W_o
+    static constexpr int N1 = (4 * D / 16) * (D / 16) / TPCH;     // W_1
+    static constexpr int N2 = (D / 16) * (4 * D / 16) / TPCH;     // W_2
     static_assert(NSLOT >= 2, "KV ring needs at least two chunks");
 };
 
@@ -152,6 +163,66 @@ __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int row
     }
 }
 
+// Consumer side of a ring chunk: wait until the producer has armed this round of the slot (a
+// parity wait can only tell a phase from its predecessor, and another warp may still own the
+// slot's previous round), then wait for the bytes.
+struct RingCtx {
+    unsigned char* ring;
+    uint64_t* bar_full;
+    uint64_t* bar_empty;
+    int* issued;
+};
+template <int NSLOT, int CHUNK_BYTES>
+__device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
+    slot = sq % NSLOT;
+    const uint32_t par = (sq / NSLOT) & 1u;
+    while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
+    mbar_wait(rc.bar_full + slot, par, 2, sq);
+    return rc.ring + (size_t)slot * CHUNK_BYTES;
+}
+__device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
+    __syncwarp();
+    if (lane == 0) mbar_arrive(rc.bar_empty + slot);
+}
+
+// GEMM over one tile of 8*NT rows with the weights taken from ring chunks (same contract as
+// gemm_rows).  Chunk j of a matrix holds TPCH consecutive 16x16 tiles of its packed image:
+// MPC whole m-tiles when K fits a chunk, else K-part (j % KSP) of m-tile j / KSP.  Warp w
+// consumes chunks w, w + NWC, ... (ring order), A fragments by conflict-free 128-bit LDS.
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, class Epi>
+__device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32_t seq0, const __nv_bfloat16* act,
+                                          int as, int warp, int lane, Epi epi) {
+    constexpr bool SPLITK = KT_TOTAL > TPCH;
+    constexpr int KSP = SPLITK ? KT_TOTAL / TPCH : 1;
+    constexpr int MPC = SPLITK ? 1 : TPCH / KT_TOTAL;
+    constexpr int KT = SPLITK ? TPCH : KT_TOTAL;
+    const int g = lane >> 2, c = lane & 3;
+    for (int j = warp; j < nchunks; j += NWC) {
+        uint32_t slot;
+        const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)j, slot)) + lane;
+#pragma unroll
+        for (int mi = 0; mi < MPC; ++mi) {
+            const int mt = SPLITK ? j / KSP : j * MPC + mi;
+            const int ks = SPLITK ? j - (j / KSP) * KSP : 0;
+            float acc[NT][4];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
+            const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                const uint4 aw = wsm[(mi * KT + kt) * 32];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
+                    mma_bf16(acc[nt], aw, lds32(p), lds32(p + 8));
+                }
+            }
+            if (mi == MPC - 1) ring_release(rc, slot, lane);
+            epi(mt, ks, acc);
+        }
+    }
+}
+
 template <int D, int DH, int NT>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
@@ -204,13 +275,30 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
+        // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
+        auto issue_weights = [&](const uint4* w, int n) {
+            const unsigned char* src = reinterpret_cast<const unsigned char*>(w);
+            for (int i0 = 0; i0 < n; i0 += VW) {
+                const int i = i0 + lane;
+                if (lane < VW && i < n) {
+                    const uint32_t sq = seq + (uint32_t)i;
+                    const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                    mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
+                    mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
+                    bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * DG::CHUNK_BYTES,
+                             (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
+                }
+                __syncwarp();
+                if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, n)));
+            }
+            seq += (uint32_t)n;
+        };
         for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
             const int b_first = unit * a.rows_per_group;
             const int n_own = min(a.rows_per_group, a.B - b_first);
-            for (int t = 1; t < N; ++t) {
+            for (int t = 0; t < N; ++t) {
                 const int cp0 = __ldg(m.chunk_ptr + t);
                 const int nch = __ldg(m.chunk_ptr + t + 1) - cp0;
-                if (nch == 0) continue;
                 const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
                 // stage this step's copy plan in shared memory (it is reused n_l * n_own times)
                 const int rp0 = __ldg(m.chunk_run_ptr + cp0);
@@ -228,9 +316,13 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 const int total = n_own * nch;
                 for (int l = 0; l < NL; ++l) {
-                    // rows < t of layer l are complete once step t-1 has appended at layer l
-                    const int need = (it * N + (t - 1)) * NL + l + 1;
-                    while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
+                    const FvLayerDev& L = m.layer[l];
+                    if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
+                    if (total > 0) {
+                        // rows < t of layer l are complete once step t-1 has appended at layer l
+                        const int need = (it * N + (t - 1)) * NL + l + 1;
+                        while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
+                    }
                     const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
                         m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
                     for (int i0 = 0; i0 < total; i0 += VW) {
@@ -264,6 +356,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, total)));
                     }
                     seq += (uint32_t)total;
+                    if (DG::WRING) {
+                        if (m.has_wo) issue_weights(L.wo, DG::NO);
+                        issue_weights(L.w1, DG::N1);
+                        issue_weights(L.w2, DG::N2);
+                    }
                 }
             }
         }
@@ -275,6 +372,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     const int rg = lane / LPR, sub = lane % LPR;
     uint32_t seq_base = 0;
     int it = 0;
+    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
     for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
         const int b_first = unit * a.rows_per_group;
         const int n_own = min(a.rows_per_group, a.B - b_first);
@@ -300,8 +398,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
                 cbar();
                 // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13) ---------------------------------
-                gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane,
-                    [&](int mt, int, float (&acc)[NT][4]) {
+                {
+                    auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                         const int f = mt * 16 + g;
                         const float b0 = __ldg(L.bqkv + f), b1 = __ldg(L.bqkv + f + 8);
 #pragma unroll
@@ -310,7 +408,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             o[0] = acc[nt][0] + b0; o[QS] = acc[nt][1] + b0;
                             o[8] = acc[nt][2] + b1; o[QS + 8] = acc[nt][3] + b1;
                         }
-                    });
+                    };
+                    if constexpr (DG::WRING) {
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
+                        seq_base += DG::NQ;
+                    } else {
+                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
+                    }
+                }
                 cbar();
                 // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) -------
                 for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
@@ -355,16 +460,10 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
                         const uint32_t sq = seq_base + (uint32_t)(FV_DEC_ORDER ? kr * GR * nch + c * nk + (r - kr * GR)
                                                                                : r * nch + c);
-                        const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                        // A parity wait can only tell a phase from its predecessor: make sure the
-                        // producer has armed THIS round of the slot before waiting on it (another
-                        // warp may still own the slot's previous round).
-                        while ((int)((uint32_t)ld_acquire_s32(sh_issued) - sq) <= 0) __nanosleep(20);
-                        mbar_wait(bar_full + slot, par, 2, sq);
-                        attend_chunk<D, DH, CH>(ring + (size_t)slot * DG::CHUNK_BYTES, min(CH, nn - c * CH), q, rg, sub,
-                                                mm, ll, acc);
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(bar_empty + slot);
+                        uint32_t slot;
+                        const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
+                        attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
+                        ring_release(rc, slot, lane);
                     }
 #pragma unroll
                     for (int o = LPR; o < 32; o <<= 1) {       // merge the RPI row groups
@@ -423,8 +522,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 // ---- optional output projection (bypassed in the paper, l.107) --------------
                 if (m.has_wo) {
-                    gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane,
-                        [&](int mt, int, float (&acc)[NT][4]) {
+                    {
+                    auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
                             const float b0 = __ldg(L.bo + f), b1 = __ldg(L.bo + f + 8);
 #pragma unroll
@@ -433,7 +532,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[0] += acc[nt][0] + b0; o[HS] += acc[nt][1] + b0;
                                 o[8] += acc[nt][2] + b1; o[HS + 8] += acc[nt][3] + b1;
                             }
-                        });
+                        };
+                    if constexpr (DG::WRING) {
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
+                        seq_base += DG::NO;
+                    } else {
+                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
+                    }
+                }
                     cbar();
                 }
                 // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
@@ -441,8 +547,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
                 cbar();
                 // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
-                gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane,
-                    [&](int mt, int, float (&acc)[NT][4]) {
+                {
+                    auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                         const int f = mt * 16 + g;
                         const float b0 = __ldg(L.b1 + f), b1 = __ldg(L.b1 + f + 8);
 #pragma unroll
@@ -453,11 +559,18 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
                             o[FS + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
                         }
-                    });
+                    };
+                    if constexpr (DG::WRING) {
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
+                        seq_base += DG::N1;
+                    } else {
+                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
+                    }
+                }
                 cbar();
                 // ---- FFN down-projection, K split KS2 ways into partial buffers -------------
-                gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane,
-                    [&](int mt, int ks, float (&acc)[NT][4]) {
+                {
+                    auto epi = [&](int mt, int ks, float (&acc)[NT][4]) {
                         const int f = mt * 16 + g;
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt) {
@@ -465,7 +578,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             o[0] = acc[nt][0]; o[HS] = acc[nt][1];
                             o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
                         }
-                    });
+                    };
+                    if constexpr (DG::WRING) {
+                        gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
+                        seq_base += DG::N2;
+                    } else {
+                        gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
+                    }
+                }
                 cbar();
                 // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
                 for (int i = tid; i < R * D; i += NWC * 32) {

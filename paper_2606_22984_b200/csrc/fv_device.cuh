@@ -61,7 +61,7 @@ struct Geo {
     static constexpr int AS = D + 8;          // bf16 activation stride (elements)
     static constexpr int QS = 3 * D + 4;      // fp32 q|k|v stride (words)
     static constexpr int FS = 4 * D + 8;      // bf16 FFN hidden stride (elements)
-    static constexpr int KS2 = (D >= 128) ? 2 : 1;   // K-splits of the W2 GEMM
+    static constexpr int KS2 = 2;             // K-splits of the W2 GEMM (= ring chunks per m-tile, fv_decode.cu)
     static constexpr size_t h_bytes = (size_t)R * HS * 4;
     static constexpr size_t a_bytes = (size_t)R * AS * 2;
     static constexpr size_t qkv_bytes = (size_t)R * QS * 4;
