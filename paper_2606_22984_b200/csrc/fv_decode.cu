@@ -30,6 +30,9 @@
 #ifndef FV_DEC_WRING
 #define FV_DEC_WRING 1      // 1: GEMM weights stream through the shared-memory ring (TMA), 0: LDG from L2
 #endif
+#ifndef FV_DEC_PREFETCH
+#define FV_DEC_PREFETCH 0   // 1: L2 prefetch of the next phase's KV runs (measured slower: 348 vs 294 ms on cfg5)
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -48,8 +51,8 @@ struct DecGeo {
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
     static constexpr size_t fixed = (G::total + 127) / 128 * 128;
-    static constexpr int TAB_C = 128, TAB_R = 320;        // per-step copy plan staged in smem
-    static constexpr size_t bar_bytes = 1024 + TAB_C * 4 + TAB_R * 8;   // 2 x 60 mbarriers, counter, plan
+    static constexpr int TAB_C = 128, TAB_R = 160;        // per-step copy plan staged in smem (x2: t, t+1)
+    static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers, counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
     static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
@@ -101,6 +104,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int wh
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// L2 prefetch of a byte range (no shared memory, no completion tracking).
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWC * 32) : "memory"); }
 __device__ __forceinline__ int ld_acquire_s32(const int* p) {
@@ -253,7 +260,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
     int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
-    int2* tab_r = reinterpret_cast<int2*>(tab_c + DG::TAB_C);
+    int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
     unsigned char* ring = smem + DG::fixed + DG::bar_bytes;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -296,27 +303,53 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
             const int b_first = unit * a.rows_per_group;
             const int n_own = min(a.rows_per_group, a.B - b_first);
-            for (int t = 0; t < N; ++t) {
+            // copy plan of a step: chunk -> run list (staged in shared memory when it fits)
+            struct Plan { int nch, nn, nruns; const int32_t* cptr; const int2* rptr; };
+            auto stage_plan = [&](int t) {
+                Plan p;
+                if (t >= N) { p.nch = p.nn = p.nruns = 0; p.cptr = nullptr; p.rptr = nullptr; return p; }
                 const int cp0 = __ldg(m.chunk_ptr + t);
-                const int nch = __ldg(m.chunk_ptr + t + 1) - cp0;
-                const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
-                // stage this step's copy plan in shared memory (it is reused n_l * n_own times)
+                p.nch = __ldg(m.chunk_ptr + t + 1) - cp0;
+                p.nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
                 const int rp0 = __ldg(m.chunk_run_ptr + cp0);
-                const int nruns = __ldg(m.chunk_run_ptr + cp0 + nch) - rp0;
-                const int32_t* cptr;
-                const int2* rptr;
+                p.nruns = __ldg(m.chunk_run_ptr + cp0 + p.nch) - rp0;
+                int32_t* tc = tab_c + (t & 1) * DG::TAB_C;
+                int2* tr = tab_r + (t & 1) * DG::TAB_R;
                 __syncwarp();
-                if (nch + 1 <= DG::TAB_C && nruns <= DG::TAB_R) {
-                    for (int i = lane; i <= nch; i += 32) tab_c[i] = __ldg(m.chunk_run_ptr + cp0 + i) - rp0;
-                    for (int i = lane; i < nruns; i += 32) tab_r[i] = __ldg(m.runs + rp0 + i);
+                if (p.nch + 1 <= DG::TAB_C && p.nruns <= DG::TAB_R) {
+                    for (int i = lane; i <= p.nch; i += 32) tc[i] = __ldg(m.chunk_run_ptr + cp0 + i) - rp0;
+                    for (int i = lane; i < p.nruns; i += 32) tr[i] = __ldg(m.runs + rp0 + i);
                     __syncwarp();
-                    cptr = tab_c; rptr = tab_r;
+                    p.cptr = tc; p.rptr = tr;
                 } else {
-                    cptr = m.chunk_run_ptr + cp0; rptr = m.runs;
+                    p.cptr = m.chunk_run_ptr + cp0; p.rptr = m.runs;      // absolute run indices
                 }
+                return p;
+            };
+            // HBM -> L2 prefetch of every KV run a later phase will copy: the ring then only has to
+            // cover the L2 -> shared memory latency, not the HBM latency.
+            auto prefetch_phase = [&](const Plan& p, int l) {
+                if (!FV_DEC_PREFETCH || p.nruns == 0 || p.rptr == m.runs) return;
+                const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
+                    m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
+                const int items = n_own * p.nruns;
+                for (int i = lane; i < items; i += 32) {
+                    const int r = i / p.nruns, j = i - r * p.nruns;
+                    const int2 run = p.rptr[j];
+                    bulk_prefetch_l2(src_l + ((size_t)r * NL * N + run.x) * DG::ROW_BYTES,
+                                     (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES);
+                }
+            };
+            Plan cur = stage_plan(0);
+            for (int t = 0; t < N; ++t) {
+                const Plan nxt = stage_plan(t + 1);
+                const int nch = cur.nch, nn = cur.nn;
+                const int32_t* cptr = cur.cptr;
+                const int2* rptr = cur.rptr;
                 const int total = n_own * nch;
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
+                    if (l + 1 < NL) prefetch_phase(cur, l + 1); else prefetch_phase(nxt, 0);
                     if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
                     if (total > 0) {
                         // rows < t of layer l are complete once step t-1 has appended at layer l
@@ -362,6 +395,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         issue_weights(L.w2, DG::N2);
                     }
                 }
+                cur = nxt;
             }
         }
         return;
