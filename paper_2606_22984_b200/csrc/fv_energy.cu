@@ -4,6 +4,7 @@
 //   F_q        : mean_b(E_b + T log q_b) and its std                    (Eq. 5)
 // All reductions use a fixed tree (shuffle, then shared memory) => bit-reproducible.
 #include "fv_internal.h"
+#include "fv_umma.cuh"
 
 namespace {
 
@@ -86,6 +87,125 @@ __global__ void __launch_bounds__(256) energy_dense_kernel(int B, int N, const i
     if (lane == 0) E[b] = -acc;
 }
 
+// Dense SK on the tensor cores (Eq. 6): T = S J as a bf16 tcgen05 GEMM with fp32
+// accumulation in tensor memory, then E_b = -1/2 sum_j T[b,j] s_bj in the epilogue.
+//   A = S  [128 samples x K = sites i], spins +-1 are exact in bf16, K-major, SWIZZLE_128B;
+//   B = J  [128 sites j  x K = sites i] (J is symmetric, so row j of J is column j), split on the
+//       fly into three bf16 terms hi + mid + lo (~24 mantissa bits: the 1e-4 relative bar needs
+//       more than bf16's 8) that accumulate into the same TMEM columns.
+// One CTA per 128 samples; j-tiles of 128 columns; per 64-wide K-block the four warps stage the
+// operand tiles in shared memory, one thread issues 4 (K = 16) MMAs per term, tcgen05.commit on
+// an mbarrier releases the tiles.  The whole GEMM is ~13 GFLOP on cfg3 (launch-latency sized), so
+// the kernel favours simplicity over overlap.
+__global__ void __launch_bounds__(128, 1) energy_dense_umma_kernel(int B, int N, const int8_t* __restrict__ spins,
+                                                                   const float* __restrict__ J, float* __restrict__ E) {
+    extern __shared__ __align__(1024) unsigned char esm_raw[];
+    unsigned char* esm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(esm_raw) + 1023) & ~(uintptr_t)1023);
+    unsigned char* sA = esm;                    // [128 x 64] bf16, 16 KB
+    unsigned char* sB = esm + 16384;            // 3 terms x [128 x 64] bf16, 48 KB
+    __shared__ uint64_t bar;
+    __shared__ uint32_t tmem_slot;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int b0 = blockIdx.x * 128;
+    if (tid == 0) { umma::mbar_init(&bar, 1); umma::fence_mbar_init(); }
+    if (warp == 0) umma::tmem_alloc<128>(&tmem_slot);
+    umma::fence_before_sync();
+    __syncthreads();
+    umma::fence_after_sync();
+    const uint32_t tmem = tmem_slot;
+    const uint32_t idesc = umma::make_idesc_bf16(128, 128);
+    const int KB = (N + 63) / 64, JT = (N + 127) / 128;
+    uint32_t phase = 0;
+    float e_acc = 0.f;
+    const int my_b = b0 + tid;                  // epilogue: thread <-> TMEM lane <-> sample
+    for (int jt = 0; jt < JT; ++jt) {
+        for (int kb = 0; kb < KB; ++kb) {
+            // ---- stage A: 128 samples x 64 sites; thread (r = tid) converts its row ------------
+            {
+                const int b = b0 + tid;
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    uint32_t w[4];
+#pragma unroll
+                    for (int h = 0; h < 4; ++h) {
+                        const int i = kb * 64 + c * 8 + 2 * h;
+                        const float x0 = (b < B && i < N) ? (float)spins[(size_t)b * N + i] : 0.f;
+                        const float x1 = (b < B && i + 1 < N) ? (float)spins[(size_t)b * N + i + 1] : 0.f;
+                        __nv_bfloat162 v = __floats2bfloat162_rn(x0, x1);
+                        w[h] = *reinterpret_cast<uint32_t*>(&v);
+                    }
+                    *reinterpret_cast<uint4*>(sA + umma::sw128_chunk(tid, c)) = make_uint4(w[0], w[1], w[2], w[3]);
+                }
+            }
+            // ---- stage B: rows j of J, 64 columns i, three bf16 split terms ----------------------
+            for (int idx = tid; idx < 128 * 8; idx += 128) {
+                const int r = idx >> 3, c = idx & 7;       // consecutive threads: consecutive 32 B of a row
+                const int j = jt * 128 + r;
+                uint32_t hi[4], mid[4], lo[4];
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    float x[2];
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        const int i = kb * 64 + c * 8 + 2 * h + q;
+                        x[q] = (j < N && i < N) ? __ldg(J + (size_t)j * N + i) : 0.f;
+                    }
+                    const __nv_bfloat16 h0 = __float2bfloat16_rn(x[0]), h1 = __float2bfloat16_rn(x[1]);
+                    const float r0 = x[0] - __bfloat162float(h0), r1 = x[1] - __bfloat162float(h1);
+                    const __nv_bfloat16 m0 = __float2bfloat16_rn(r0), m1 = __float2bfloat16_rn(r1);
+                    const __nv_bfloat16 l0 = __float2bfloat16_rn(r0 - __bfloat162float(m0));
+                    const __nv_bfloat16 l1 = __float2bfloat16_rn(r1 - __bfloat162float(m1));
+                    __nv_bfloat162 vh(h0, h1), vm(m0, m1), vl(l0, l1);
+                    hi[h] = *reinterpret_cast<uint32_t*>(&vh);
+                    mid[h] = *reinterpret_cast<uint32_t*>(&vm);
+                    lo[h] = *reinterpret_cast<uint32_t*>(&vl);
+                }
+                const uint32_t off = umma::sw128_chunk(r, c);
+                *reinterpret_cast<uint4*>(sB + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                *reinterpret_cast<uint4*>(sB + 16384 + off) = make_uint4(mid[0], mid[1], mid[2], mid[3]);
+                *reinterpret_cast<uint4*>(sB + 32768 + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            }
+            umma::fence_smem_to_async();
+            __syncthreads();
+            if (tid == 0) {
+                umma::fence_after_sync();
+                const uint32_t a0 = umma::smem_u32(sA), bb = umma::smem_u32(sB);
+#pragma unroll
+                for (int term = 0; term < 3; ++term) {
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks) {
+                        umma::mma_bf16_ss(tmem, umma::make_desc_sw128(a0 + ks * 32),
+                                          umma::make_desc_sw128(bb + term * 16384 + ks * 32), idesc,
+                                          (kb | term | ks) != 0);
+                    }
+                }
+                umma::commit(&bar);
+            }
+            umma::mbar_wait(&bar, phase);          // MMAs done: tiles may be overwritten, TMEM readable
+            phase ^= 1;
+        }
+        // ---- epilogue of this j-tile: E_b += sum_j T[b,j] s_bj ------------------------------------
+        umma::fence_after_sync();
+#pragma unroll 1
+        for (int cb = 0; cb < 4; ++cb) {
+            float v[32];
+            umma::tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + cb * 32, v);
+            if (my_b < B) {
+#pragma unroll
+                for (int q = 0; q < 32; ++q) {
+                    const int j = jt * 128 + cb * 32 + q;
+                    if (j < N) e_acc += v[q] * (float)spins[(size_t)my_b * N + j];
+                }
+            }
+        }
+        umma::fence_before_sync();
+        __syncthreads();                            // all TMEM reads done before the next tile's MMAs
+    }
+    if (my_b < B) E[my_b] = -0.5f * e_acc;
+    __syncthreads();
+    if (warp == 0) umma::tmem_dealloc<128>(tmem);
+}
+
 __global__ void __launch_bounds__(1024) free_energy_kernel(int B, const float* __restrict__ E,
                                                            const float* __restrict__ logq, double T,
                                                            double* __restrict__ out) {
@@ -119,6 +239,17 @@ cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_
 }
 
 cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const float* J, float* E, cudaStream_t s) {
+    if (N >= 32) {                                  // tensor-core s^T J s (tcgen05, 3-term bf16 split of J)
+        const int smem_tc = 65536 + 1024;
+        static bool attr_set = false;
+        if (!attr_set) {
+            cudaError_t e = cudaFuncSetAttribute(energy_dense_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_tc);
+            if (e != cudaSuccess) return e;
+            attr_set = true;
+        }
+        energy_dense_umma_kernel<<<(B + 127) / 128, 128, smem_tc, s>>>(B, N, spins, J, E);
+        return cudaGetLastError();
+    }
     const size_t smem = (size_t)8 * N;
     if (smem > 200 * 1024) return cudaErrorInvalidValue;
     if (smem > 48 * 1024) cudaFuncSetAttribute(energy_dense_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
