@@ -17,6 +17,8 @@ struct fv_model {
     void* arena = nullptr;       // all read-only parameters, one allocation
     size_t arena_bytes = 0;
     size_t kv_bytes = 0;
+    void* ws = nullptr;          // fv_log_prob workspace (h, q)
+    size_t ws_bytes = 0;
     int n_sms = 0;
     int device = 0;
 };
@@ -130,7 +132,10 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     m->n_sms = prop.multiProcessorCount;
     m->device = dev;
     Arena A;
-    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b; };
+    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn; };
+    const bool lp_tc = !cfg->has_wo && (d == 32 || d == 64 || d == 128);   // fv_logprob.cu path
+    const int KP = d < 64 ? 64 : d;
+    std::vector<uint16_t> img((size_t)std::max(3 * d * KP, (f / 128) * (128 * KP + d * 128)));
     std::vector<Off> off(NL);
     const float* w = weights;
     const size_t o_tok = A.put(w, sizeof(float) * 2 * cfg->d_token);
@@ -147,6 +152,11 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         }
         pack_mma_a(tmp.data(), 3 * d, d, pk.data());
         o.wqkv = A.put(pk.data(), (size_t)3 * d * d * 2);
+        o.img_qkv = o.img_ffn = 0;
+        if (lp_tc) {
+            fv_pack_sw128(tmp.data(), 3 * d, d, d, KP, img.data());
+            o.img_qkv = A.put(img.data(), (size_t)3 * d * KP * 2);
+        }
         o.bqkv = A.put(tb.data(), 4 * 3 * d);
         o.wo = o.bo = 0;
         if (cfg->has_wo) {
@@ -156,7 +166,18 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         }
         o.ln2g = A.put(w, 4 * d); w += d;
         o.ln2b = A.put(w, 4 * d); w += d;
-        pack_mma_a(w, f, d, pk.data()); w += (size_t)f * d;
+        pack_mma_a(w, f, d, pk.data());
+        if (lp_tc) {                                  // per 128-column hidden chunk: W1_j | W2_j
+            const float* W1 = w;
+            const float* W2 = w + (size_t)f * d + f;   // after W1 and b1
+            const size_t per = (size_t)128 * KP + (size_t)d * 128;
+            for (int j = 0; j < f / 128; ++j) {
+                fv_pack_sw128(W1 + (size_t)j * 128 * d, 128, d, d, KP, img.data() + j * per);
+                fv_pack_sw128(W2 + (size_t)j * 128, d, 128, f, 128, img.data() + j * per + (size_t)128 * KP);
+            }
+            o.img_ffn = A.put(img.data(), (size_t)(f / 128) * per * 2);
+        }
+        w += (size_t)f * d;
         o.w1 = A.put(pk.data(), (size_t)f * d * 2);
         o.b1 = A.put(w, 4 * f); w += f;
         pack_mma_a(w, d, f, pk.data()); w += (size_t)d * f;
@@ -200,10 +221,15 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     void* kv = nullptr;
     e = cudaMalloc(&kv, m->kv_bytes);
     if (e != cudaSuccess) { cudaFree(m->arena); delete m; return cuda_fail(e, "cudaMalloc(KV pool)"); }
+    if (lp_tc) {                                      // fv_log_prob workspace: h and q, fp32 [max_batch * N, d]
+        m->ws_bytes = (size_t)2 * cfg->max_batch * N * d * sizeof(float);
+        e = cudaMalloc(&m->ws, m->ws_bytes);
+        if (e != cudaSuccess) { cudaFree(kv); cudaFree(m->arena); delete m; return cuda_fail(e, "cudaMalloc(log_prob workspace)"); }
+    }
     cudaStream_t s = (cudaStream_t)stream;
     e = cudaMemcpyAsync(m->arena, A.host.data(), m->arena_bytes, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) { cudaFree(kv); cudaFree(m->arena); delete m; return cuda_fail(e, "parameter upload"); }
+    if (e != cudaSuccess) { cudaFree(kv); cudaFree(m->ws); cudaFree(m->arena); delete m; return cuda_fail(e, "parameter upload"); }
 
     unsigned char* base = (unsigned char*)m->arena;
     FvModelDev& D = m->dev;
@@ -219,6 +245,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.chunk_run_ptr = (const int32_t*)(base + o_crp);
     D.runs = (const int2*)(base + o_runs);
     D.kv = (__nv_bfloat16*)kv;
+    D.lp_h = (float*)m->ws;
+    D.lp_q = m->ws ? (float*)m->ws + (size_t)cfg->max_batch * N * d : nullptr;
     for (int l = 0; l < NL; ++l) {
         const Off& o = off[l];
         FvLayerDev& L = D.layer[l];
@@ -232,6 +260,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         L.b2 = (const float*)(base + o.b2);
         L.ln1_g = (const float*)(base + o.ln1g); L.ln1_b = (const float*)(base + o.ln1b);
         L.ln2_g = (const float*)(base + o.ln2g); L.ln2_b = (const float*)(base + o.ln2b);
+        L.img_qkv = lp_tc ? base + o.img_qkv : nullptr;
+        L.img_ffn = lp_tc ? base + o.img_ffn : nullptr;
     }
     *out = m;
     return FV_OK;
@@ -241,6 +271,7 @@ void fv_destroy_model(fv_model* m) {
     if (!m) return;
     cudaDeviceSynchronize();
     cudaFree(m->dev.kv);
+    cudaFree(m->ws);
     cudaFree(m->arena);
     delete m;
 }
@@ -279,6 +310,15 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {
     if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
     if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
+    const char* force = std::getenv("FLASHVAN_LOGPROB");          // "chunked": the persistent teacher-forcing kernel
+    if (!(force && std::strcmp(force, "chunked") == 0)) {
+        int n_launch = 0;
+        cudaError_t e2 = fv_launch_logprob_tc(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B, spins, logq,
+                                              cond_p, m->n_sms, &n_launch, (cudaStream_t)stream);
+        if (e2 == cudaSuccess) { g_launches += n_launch; return FV_OK; }
+        if (e2 != cudaErrorNotSupported) return cuda_fail(e2, "fv_log_prob launch");
+        (void)cudaGetLastError();
+    }
     FvForwardArgs a{};
     a.mode = FV_MODE_LOGPROB;
     a.B = B;

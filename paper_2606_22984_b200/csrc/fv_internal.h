@@ -22,6 +22,9 @@ struct FvLayerDev {
     const uint4* w2;    // [d, 4d]
     const float *bqkv, *bo, *b1, *b2;
     const float *ln1_g, *ln1_b, *ln2_g, *ln2_b;
+    // fv_logprob.cu: pre-swizzled (SWIZZLE_128B, K-major) bf16 images, copied verbatim into shared memory
+    const unsigned char* img_qkv;   // [3d rows x KP]
+    const unsigned char* img_ffn;   // per 128-column hidden chunk j: W1_j [128 x KP] | W2_j [d x 128]
 };
 
 struct FvModelDev {
@@ -41,6 +44,8 @@ struct FvModelDev {
     const int32_t* chunk_run_ptr;  // [n_chunks+1]
     const int2* runs;
     __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16)
+    float* lp_h;            // fv_log_prob workspace: residual stream [max_batch * N, d] fp32 (or nullptr)
+    float* lp_q;            //                        queries of the current layer, same shape
     FvLayerDev layer[FV_MAX_LAYERS];
 };
 
@@ -65,6 +70,9 @@ cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int 
 size_t fv_forward_smem_bytes(int d_model, int nt);
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt,
                              const FvForwardArgs& a, int grid, cudaStream_t s);
+cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
+                                 float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s);
+void fv_pack_sw128(const float* W, int rows, int K, int ld, int KP, uint16_t* dst);
 cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_t* rowptr,
                                  const int32_t* col, const float* val, int integer, float* E,
                                  cudaStream_t s);
