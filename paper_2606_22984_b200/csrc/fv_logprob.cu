@@ -65,6 +65,19 @@ __device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __re
     }
 }
 
+constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
+
+template <int E> __device__ __forceinline__ void ld_row(const float* p, float (&x)[E]) {
+    if constexpr (E == 4) { const float4 v = *reinterpret_cast<const float4*>(p); x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
+    else if constexpr (E == 2) { const float2 v = *reinterpret_cast<const float2*>(p); x[0] = v.x; x[1] = v.y; }
+    else { x[0] = *p; }
+}
+template <int E> __device__ __forceinline__ void st_row(float* p, const float (&x)[E]) {
+    if constexpr (E == 4) *reinterpret_cast<float4*>(p) = make_float4(x[0], x[1], x[2], x[3]);
+    else if constexpr (E == 2) *reinterpret_cast<float2*>(p) = make_float2(x[0], x[1]);
+    else *p = x[0];
+}
+
 struct LpArgs {
     int32_t B, N, NL, layer, d_token, ln2_style;
     float ln_eps;
@@ -118,30 +131,39 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     uint32_t ph = 0;
     bool w_ready = false;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        // ---- prologue: (embedding) + LN1 -> bf16 A tile ---------------------------------------
-        for (int r = warp; r < TM; r += LP_THREADS / 32) {
-            const long long gi = tile * TM + r;
-            float x[E];
-            if (gi < a.M) {
-                if (a.layer == 0) {                 // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
-                    const int t = (int)(gi % a.N);
-                    const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
+        // ---- prologue: (embedding) + LN1 -> bf16 A tile.  A warp owns 16 rows; their loads are
+        //      issued RB rows at a time before any arithmetic (one HBM round trip per batch) ------
+        for (int rb = 0; rb < TM / (LP_THREADS / 32); rb += RB) {
+            float x[RB][E];
 #pragma unroll
-                    for (int j = 0; j < E; ++j) {
-                        const int f = lane * E + j;
-                        x[j] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
-                                             : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
-                        a.h[gi * D + f] = x[j];
+            for (int u = 0; u < RB; ++u) {
+                const int r = warp + (rb + u) * (LP_THREADS / 32);
+                const long long gi = tile * TM + r;
+                if (gi < a.M) {
+                    if (a.layer == 0) {             // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
+                        const int t = (int)(gi % a.N);
+                        const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
+#pragma unroll
+                        for (int j = 0; j < E; ++j) {
+                            const int f = lane * E + j;
+                            x[u][j] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
+                                                    : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
+                        }
+                    } else {
+                        ld_row<E>(a.h + gi * D + lane * E, x[u]);
                     }
                 } else {
 #pragma unroll
-                    for (int j = 0; j < E; ++j) x[j] = a.h[gi * D + lane * E + j];
+                    for (int j = 0; j < E; ++j) x[u][j] = 0.f;
                 }
-            } else {
-#pragma unroll
-                for (int j = 0; j < E; ++j) x[j] = 0.f;
             }
-            ln_to_tile<D>(x, a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
+#pragma unroll
+            for (int u = 0; u < RB; ++u) {
+                const int r = warp + (rb + u) * (LP_THREADS / 32);
+                const long long gi = tile * TM + r;
+                if (a.layer == 0 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
+                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
+            }
         }
         umma::fence_smem_to_async();
         __syncthreads();
@@ -283,15 +305,23 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
     long long gch = 0;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         // ---- prologue: LN2 -> bf16 A tile (ln2_style 1: the residual stream becomes LN2(h)) -----
-        for (int r = warp; r < TM; r += LP_THREADS / 32) {
-            const long long gi = tile * TM + r;
-            float x[E];
+        for (int rb = 0; rb < TM / (LP_THREADS / 32); rb += RB) {
+            float x[RB][E];
 #pragma unroll
-            for (int j = 0; j < E; ++j) x[j] = gi < a.M ? a.h[gi * D + lane * E + j] : 0.f;
-            ln_to_tile<D>(x, a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
-            if (a.ln2_style == 1 && gi < a.M) {
+            for (int u = 0; u < RB; ++u) {
+                const long long gi = tile * TM + warp + (rb + u) * (LP_THREADS / 32);
+                if (gi < a.M) ld_row<E>(a.h + gi * D + lane * E, x[u]);
+                else {
 #pragma unroll
-                for (int j = 0; j < E; ++j) a.h[gi * D + lane * E + j] = x[j];
+                    for (int j = 0; j < E; ++j) x[u][j] = 0.f;
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < RB; ++u) {
+                const int r = warp + (rb + u) * (LP_THREADS / 32);
+                const long long gi = tile * TM + r;
+                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
+                if (a.ln2_style == 1 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
             }
         }
         umma::fence_smem_to_async();
