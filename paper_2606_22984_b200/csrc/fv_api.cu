@@ -210,6 +210,32 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         chunk_ptr[t + 1] = (int32_t)chunk_run_ptr.size() - 1;
     }
     if (runs.empty()) runs.push_back(make_int2(0, 0));
+    // block attention plan of fv_logprob.cu: union of the key positions of 32 consecutive mask rows
+    const int BQ = 32;
+    const int n_blk = (N + BQ - 1) / BQ;
+    std::vector<int32_t> blk_uptr(1, 0), ukeys;
+    std::vector<uint16_t> amask;
+    for (int blk = 0; blk < n_blk; ++blk) {
+        const int t0 = blk * BQ, t1 = std::min(N, t0 + BQ);
+        std::vector<int32_t> u;
+        for (int t = t0; t < t1; ++t) u.insert(u.end(), mask_col + mask_rowptr[t], mask_col + mask_rowptr[t + 1]);
+        std::sort(u.begin(), u.end());
+        u.erase(std::unique(u.begin(), u.end()), u.end());
+        const size_t n_real = u.size();
+        while (u.size() % 16) u.push_back(0);             // padding keys: a valid row, never allowed
+        const size_t base = amask.size();
+        amask.resize(base + u.size() / 16 * BQ, 0);
+        for (int t = t0; t < t1; ++t)
+            for (int e = mask_rowptr[t]; e < mask_rowptr[t + 1]; ++e) {
+                const size_t k = std::lower_bound(u.begin(), u.begin() + n_real, mask_col[e]) - u.begin();
+                amask[base + (k / 16) * BQ + (t - t0)] |= (uint16_t)(1u << (k % 16));
+            }
+        ukeys.insert(ukeys.end(), u.begin(), u.end());
+        blk_uptr.push_back((int32_t)ukeys.size());
+    }
+    const size_t o_bu = A.put(blk_uptr.data(), sizeof(int32_t) * blk_uptr.size());
+    const size_t o_uk = A.put(ukeys.data(), sizeof(int32_t) * ukeys.size());
+    const size_t o_am = A.put(amask.data(), sizeof(uint16_t) * amask.size());
     const size_t o_cp = A.put(chunk_ptr.data(), sizeof(int32_t) * chunk_ptr.size());
     const size_t o_crp = A.put(chunk_run_ptr.data(), sizeof(int32_t) * chunk_run_ptr.size());
     const size_t o_runs = A.put(runs.data(), sizeof(int2) * runs.size());
@@ -244,6 +270,10 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.chunk_ptr = (const int32_t*)(base + o_cp);
     D.chunk_run_ptr = (const int32_t*)(base + o_crp);
     D.runs = (const int2*)(base + o_runs);
+    D.att_blk_uptr = (const int32_t*)(base + o_bu);
+    D.att_ukeys = (const int32_t*)(base + o_uk);
+    D.att_mask = (const uint16_t*)(base + o_am);
+    D.att_nblk = n_blk;
     D.kv = (__nv_bfloat16*)kv;
     D.lp_h = (float*)m->ws;
     D.lp_q = m->ws ? (float*)m->ws + (size_t)cfg->max_batch * N * d : nullptr;

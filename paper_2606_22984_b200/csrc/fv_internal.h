@@ -44,6 +44,12 @@ struct FvModelDev {
     const int32_t* chunk_run_ptr;  // [n_chunks+1]
     const int2* runs;
     __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16)
+    // fv_logprob.cu block attention plan: per block of 32 queries the padded union of key positions and,
+    // per 16-key step and query, a 16-bit allow mask
+    const int32_t* att_blk_uptr;   // [att_nblk + 1] offsets into att_ukeys (multiples of 16)
+    const int32_t* att_ukeys;
+    const uint16_t* att_mask;      // [(total keys / 16) * 32]
+    int32_t att_nblk;
     float* lp_h;            // fv_log_prob workspace: residual stream [max_batch * N, d] fp32 (or nullptr)
     float* lp_q;            //                        queries of the current layer, same shape
     FvLayerDev layer[FV_MAX_LAYERS];

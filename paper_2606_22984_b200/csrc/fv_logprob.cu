@@ -11,6 +11,7 @@
 // and lp_head_kernel: sigmoid head, log p of the given spin, per-sample fp64 sum (Alg. 1 l.8-9).
 // GEMM operands are bf16 with fp32 accumulation; LayerNorm, softmax, residual stream stay fp32 --
 // the same arithmetic as the decode kernel, so both paths agree with the oracle inside one bound.
+#include <cstdlib>
 #include <cstring>
 
 #include "fv_device.cuh"
@@ -255,6 +256,195 @@ __global__ void __launch_bounds__(512) lp_attn_kernel(const __grid_constant__ Lp
     }
 }
 
+// --------------------------------------------------------------------------------- attention (tensor cores)
+// Block-skipping masked attention for d_h = 16 (all BASELINE configs).  A CTA owns BQ = 32
+// consecutive positions of one sample, one warp per head.  The host plan (fv_create_model) gives,
+// per query block, the sorted UNION of the key positions its 32 mask rows name (padded to 16) and,
+// per 16-key step and query, a 16-bit allow mask: key tiles outside the union are never loaded,
+// steps in which none of a warp's 16 queries has an allowed key are skipped, and inside a step
+// masked-out scores get probability exactly 0.
+//   S = Q K^T : mma.sync m16n8k16 (k = d_h = 16: one MMA per 8 keys), Q pre-scaled; Q and P enter as
+//               bf16 hi + lo pairs (two MMAs), so only K and V carry bf16 rounding -- as in fv_sample
+//   online softmax (base 2, fp32) on the C fragments
+//   O += P V  : P re-used from the C fragments as the A operand (bf16), V via ldmatrix.trans
+// K|V rows of the union are staged in shared memory by cp.async in chunks of 64 keys, double
+// buffered; rows are padded by 16 B so the 8 rows of an ldmatrix tile hit different banks.
+constexpr int ATT_BQ = 32, ATT_UC = 64;
+
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// (x, y) -> packed bf16 pairs hi and lo with hi + lo = (x, y) to ~16 mantissa bits
+__device__ __forceinline__ void split_bf16(float x, float y, uint32_t& hi, uint32_t& lo) {
+    const __nv_bfloat16 hx = __float2bfloat16_rn(x), hy = __float2bfloat16_rn(y);
+    __nv_bfloat162 h(hx, hy);
+    hi = *reinterpret_cast<uint32_t*>(&h);
+    lo = pack_bf16(x - __bfloat162float(hx), y - __bfloat162float(hy));
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src) : "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_constant__ LpArgs a,
+                                                                  const int32_t* __restrict__ blk_uptr,
+                                                                  const int32_t* __restrict__ ukeys,
+                                                                  const uint16_t* __restrict__ amask, int n_blk) {
+    constexpr int NTH = D / 16 * 32, RS = 4 * D + 16, BUF = ATT_UC * RS, PCS = 4 * D / 16;   // 16-B pieces per row
+    extern __shared__ __align__(16) unsigned char att_sm[];
+    const int tid = threadIdx.x, head = tid >> 5, lane = tid & 31, g = lane >> 2, c = lane & 3;
+    const int b = blockIdx.x / n_blk, blk = blockIdx.x - b * n_blk;
+    const int t0 = blk * ATT_BQ;
+    const int u0 = __ldg(blk_uptr + blk), U = __ldg(blk_uptr + blk + 1) - u0;
+    const int n_chunks = (U + ATT_UC - 1) / ATT_UC;
+    const unsigned char* kvb = reinterpret_cast<const unsigned char*>(a.kv + ((size_t)b * a.NL + a.layer) * a.N * (2 * D));
+    const uint32_t sm0 = umma::smem_u32(att_sm);
+    auto stage = [&](int ch) {
+        const int k0 = ch * ATT_UC, nk = min(ATT_UC, U - k0);
+        const uint32_t dst = sm0 + (ch & 1) * BUF;
+        for (int i = tid; i < nk * PCS; i += NTH) {
+            const int r = i / PCS, pc = i - r * PCS;
+            const int key = __ldg(ukeys + u0 + k0 + r);
+            cp_async16(dst + r * RS + pc * 16, kvb + (size_t)key * (4 * D) + pc * 16);
+        }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+    };
+    stage(0);
+    // Q fragments (A operand), pre-scaled by log2(e)/sqrt(d_h)
+    const float qs = kLog2e * 0.25f;
+    uint32_t qa[2][4], ql[2][4];        // bf16 hi and lo parts: q keeps ~16 mantissa bits through the MMA
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int t = t0 + mt * 16 + g + hh * 8;
+            float2 lo = make_float2(0.f, 0.f), hi = lo;
+            if (t < a.N) {
+                const float* qp = a.q + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
+                lo = *reinterpret_cast<const float2*>(qp);
+                hi = *reinterpret_cast<const float2*>(qp + 8);
+            }
+            split_bf16(lo.x * qs, lo.y * qs, qa[mt][hh], ql[mt][hh]);
+            split_bf16(hi.x * qs, hi.y * qs, qa[mt][hh + 2], ql[mt][hh + 2]);
+        }
+    }
+    float o[2][2][4], mrow[2][2], lrow[2][2];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+            mrow[mt][x] = -1e30f; lrow[mt][x] = 0.f;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) o[mt][x][e] = 0.f;
+        }
+    const uint16_t* mk = amask + (size_t)(u0 / 16) * ATT_BQ;
+    for (int ch = 0; ch < n_chunks; ++ch) {
+        if (ch + 1 < n_chunks) { stage(ch + 1); asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+        else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+        __syncthreads();
+        const uint32_t buf = sm0 + (ch & 1) * BUF;
+        const int nst = (min(ATT_UC, U - ch * ATT_UC)) / 16;
+        for (int st = 0; st < nst; ++st) {
+            const uint16_t* ms = mk + (size_t)(ch * (ATT_UC / 16) + st) * ATT_BQ;
+            uint32_t bits[2][2];
+            bool any[2];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                bits[mt][0] = __ldg(ms + mt * 16 + g);
+                bits[mt][1] = __ldg(ms + mt * 16 + g + 8);
+                any[mt] = __any_sync(0xffffffffu, (bits[mt][0] | bits[mt][1]) != 0);
+            }
+            if (!any[0] && !any[1]) continue;
+            uint32_t kf[4], vf[4];
+            {
+                const int mi = lane >> 3, rr = lane & 7;
+                ldsm_x4(kf, buf + (st * 16 + (mi >> 1) * 8 + rr) * RS + head * 32 + (mi & 1) * 16);
+                ldsm_x4_t(vf, buf + (st * 16 + (mi & 1) * 8 + rr) * RS + 2 * D + head * 32 + (mi >> 1) * 16);
+            }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                if (!any[mt]) continue;
+                float sc[2][4];
+#pragma unroll
+                for (int n = 0; n < 2; ++n) {
+                    sc[n][0] = sc[n][1] = sc[n][2] = sc[n][3] = 0.f;
+                    mma_bf16(sc[n], make_uint4(qa[mt][0], qa[mt][1], qa[mt][2], qa[mt][3]), kf[2 * n], kf[2 * n + 1]);
+                    mma_bf16(sc[n], make_uint4(ql[mt][0], ql[mt][1], ql[mt][2], ql[mt][3]), kf[2 * n], kf[2 * n + 1]);
+                }
+                bool ok[2][4];
+                float mx[2] = {mrow[mt][0], mrow[mt][1]};
+#pragma unroll
+                for (int n = 0; n < 2; ++n)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        ok[n][e] = (bits[mt][e >> 1] >> (n * 8 + 2 * c + (e & 1))) & 1u;
+                        if (ok[n][e]) mx[e >> 1] = fmaxf(mx[e >> 1], sc[n][e]);
+                    }
+#pragma unroll
+                for (int x = 0; x < 2; ++x) {
+                    mx[x] = fmaxf(mx[x], __shfl_xor_sync(0xffffffffu, mx[x], 1));
+                    mx[x] = fmaxf(mx[x], __shfl_xor_sync(0xffffffffu, mx[x], 2));
+                }
+                float corr[2];
+#pragma unroll
+                for (int x = 0; x < 2; ++x) {
+                    corr[x] = exp2f(mrow[mt][x] - mx[x]);
+                    mrow[mt][x] = mx[x];
+                    lrow[mt][x] *= corr[x];
+                }
+                float p[2][4];
+#pragma unroll
+                for (int n = 0; n < 2; ++n)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        p[n][e] = ok[n][e] ? exp2f(sc[n][e] - mx[e >> 1]) : 0.f;
+                        lrow[mt][e >> 1] += p[n][e];
+                    }
+#pragma unroll
+                for (int x = 0; x < 2; ++x)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) o[mt][x][e] *= corr[e >> 1];
+                uint4 pa, pl;                              // P = hi + lo in bf16 (as q above)
+                split_bf16(p[0][0], p[0][1], pa.x, pl.x);
+                split_bf16(p[0][2], p[0][3], pa.y, pl.y);
+                split_bf16(p[1][0], p[1][1], pa.z, pl.z);
+                split_bf16(p[1][2], p[1][3], pa.w, pl.w);
+                mma_bf16(o[mt][0], pa, vf[0], vf[1]);
+                mma_bf16(o[mt][1], pa, vf[2], vf[3]);
+                mma_bf16(o[mt][0], pl, vf[0], vf[1]);
+                mma_bf16(o[mt][1], pl, vf[2], vf[3]);
+            }
+        }
+        __syncthreads();                               // buffer (ch & 1) is restaged two chunks later
+    }
+    // finalise: h += O / l  (Alg. 2 l.15: residual without W_O)
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            float l = lrow[mt][hh];
+            l += __shfl_xor_sync(0xffffffffu, l, 1);
+            l += __shfl_xor_sync(0xffffffffu, l, 2);
+            const int t = t0 + mt * 16 + g + hh * 8;
+            if (t < a.N && l > 0.f) {
+                const float inv = 1.0f / l;
+                float* hp = a.h + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
+#pragma unroll
+                for (int x = 0; x < 2; ++x) {
+                    float2 hv = *reinterpret_cast<float2*>(hp + x * 8);
+                    hv.x += o[mt][x][hh * 2] * inv;
+                    hv.y += o[mt][x][hh * 2 + 1] * inv;
+                    *reinterpret_cast<float2*>(hp + x * 8) = hv;
+                }
+            }
+        }
+}
+
 // --------------------------------------------------------------------------------- FFN
 // h <- h + W2 gelu(W1 LN2(h) + b1) + b2 for a tile of 128 rows (Alg. 2 l.16 form; ln2_style 1:
 // h <- LN2(h) first, Alg. 1 l.5).  The hidden layer is processed in chunks of HC = 128 columns:
@@ -454,10 +644,13 @@ template <int D, int DH>
 cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* logq, float* cond_p, int n_sms,
                       cudaStream_t s) {
     using G = LpGeo<D>;
+    constexpr int att_smem = 2 * ATT_UC * (4 * D + 16);
+    static const bool fv_lp_attn_alu = [] { const char* v = std::getenv("FLASHVAN_ATTN"); return v && std::strcmp(v, "alu") == 0; }();
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(lp_qkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::QKV_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_ffn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::FFN_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_attn_mma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -473,8 +666,13 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
         a.layer = l;
         a.w_img = L.img_qkv; a.bias = L.bqkv; a.bias2 = nullptr; a.ln_g = L.ln1_g; a.ln_b = L.ln1_b;
         lp_qkv_kernel<D><<<grid, LP_THREADS, G::QKV_SMEM, s>>>(a);
-        lp_attn_kernel<D, DH><<<(unsigned)((a.M + rows_per_cta - 1) / rows_per_cta), 512, 0, s>>>(a, m.mask_rowptr, m.mask_col,
-                                                                                            rows_per_cta);
+        if (DH == 16 && m.att_nblk > 0 && !fv_lp_attn_alu) {
+            lp_attn_mma_kernel<D><<<(unsigned)(B * m.att_nblk), D / 16 * 32, att_smem, s>>>(a, m.att_blk_uptr, m.att_ukeys,
+                                                                                           m.att_mask, m.att_nblk);
+        } else {
+            lp_attn_kernel<D, DH><<<(unsigned)((a.M + rows_per_cta - 1) / rows_per_cta), 512, 0, s>>>(a, m.mask_rowptr, m.mask_col,
+                                                                                                rows_per_cta);
+        }
         a.w_img = L.img_ffn; a.bias = L.b1; a.bias2 = L.b2; a.ln_g = L.ln2_g; a.ln_b = L.ln2_b;
         lp_ffn_kernel<D><<<grid, LP_THREADS, G::FFN_SMEM, s>>>(a);
     }
