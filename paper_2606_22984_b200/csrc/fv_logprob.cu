@@ -20,7 +20,8 @@
 namespace {
 using namespace fvdev;
 
-constexpr int LP_THREADS = 256;   // 8 warps: warp w reads TMEM lanes 32 (w % 4) .. +31, column half w / 4
+constexpr int LP_THREADS = 512;   // 16 warps: warp w reads TMEM lanes 32 (w % 4) .. +31, column group w / 4
+constexpr int NCG = LP_THREADS / 128;   // column groups sharing one TMEM lane quarter
 constexpr int TM = 128;           // rows per tile = UMMA M
 
 template <int D> struct LpGeo {
@@ -43,11 +44,24 @@ template <int D> struct LpGeo {
     static constexpr int TMEM_F = (HC + D) <= 256 ? 256 : 512;
 };
 
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ void sts64(uint32_t addr, uint32_t x, uint32_t y) {
+    asm volatile("st.shared.v2.b32 [%0], {%1,%2};\n" ::"r"(addr), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t x) {
+    asm volatile("st.shared.b32 [%0], %1;\n" ::"r"(addr), "r"(x) : "memory");
+}
+__device__ __forceinline__ void sts16(uint32_t addr, uint16_t x) {
+    asm volatile("st.shared.b16 [%0], %1;\n" ::"r"(addr), "h"(x) : "memory");
+}
+
 // LayerNorm of one fp32 row (values already in registers, E = D/32 per lane, feature lane*E + j)
 // -> bf16 into the swizzled A tile row `r`.  Returns the normalised values in x (for ln2_style 1).
 template <int D>
 __device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __restrict__ gam, const float* __restrict__ bet,
-                                           float eps, unsigned char* sA, int r, int lane) {
+                                           float eps, uint32_t sA, int r, int lane) {
     constexpr int E = D / 32;
     float s = 0.f;
 #pragma unroll
@@ -61,9 +75,30 @@ __device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __re
     for (int j = 0; j < E; ++j) {
         const int f = lane * E + j;
         x[j] = (x[j] - mean) * rstd * __ldg(gam + f) + __ldg(bet + f);
-        const int kb = f >> 6, c = (f & 63) >> 3, e = f & 7;
-        *reinterpret_cast<__nv_bfloat16*>(sA + kb * (TM * 128) + umma::sw128_chunk(r, c) + e * 2) = __float2bfloat16_rn(x[j]);
     }
+    // the lane's E consecutive features sit inside one 16-byte chunk of the swizzled row
+    const int f0 = lane * E;
+    const uint32_t dst = sA + (f0 >> 6) * (TM * 128) + umma::sw128_chunk(r, (f0 & 63) >> 3) + (f0 & 7) * 2;
+    if constexpr (E == 4) sts64(dst, pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]));
+    else if constexpr (E == 2) sts32(dst, pack_bf16(x[0], x[1]));
+    else { const __nv_bfloat16 v = __float2bfloat16_rn(x[0]); sts16(dst, *reinterpret_cast<const uint16_t*>(&v)); }
+}
+
+// Exact-GELU 0.5 x (1 + erf(x / sqrt 2)) with erf from Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7,
+// far below the bf16 rounding of the result): one rcp.approx, one ex2.approx, six FMAs -- the
+// epilogue of the fused FFN evaluates 4d of these per row and bounds the kernel.
+__device__ __forceinline__ float gelu_fast(float x) {
+    const float z = fabsf(x) * 0.70710678118654752f;
+    float t;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, z, 1.0f)));
+    float p = fmaf(1.061405429f, t, -1.453152027f);
+    p = fmaf(p, t, 1.421413741f);
+    p = fmaf(p, t, -0.284496736f);
+    p = fmaf(p, t, 0.254829592f);
+    float ex;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(-z * z * kLog2e));
+    const float e = fmaf(-p * t, ex, 1.0f);                     // erf(|x| / sqrt 2)
+    return 0.5f * x + 0.5f * fabsf(x) * e;                      // 0.5 x (1 + sign(x) e)
 }
 
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
@@ -104,6 +139,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(lp_raw) + 1023) & ~(uintptr_t)1023);
     unsigned char* sA = sm;
     unsigned char* sW = sm + G::A_BYTES;
+    const uint32_t sA_u32 = umma::smem_u32(sA);
     __shared__ uint64_t bar_w, bar_mma;
     __shared__ uint32_t tmem_slot;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -163,7 +199,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
                 const int r = warp + (rb + u) * (LP_THREADS / 32);
                 const long long gi = tile * TM + r;
                 if (a.layer == 0 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
-                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
+                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
             }
         }
         umma::fence_smem_to_async();
@@ -196,7 +232,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
             const int b = ok ? (int)(gi / a.N) : 0, t = ok ? (int)(gi % a.N) : 0;
             float* qrow = a.q + gi * D;
             __nv_bfloat16* kvrow = a.kv + (((size_t)b * a.NL + a.layer) * a.N + t) * (2 * D);
-            for (int cb = (warp >> 2); cb < G::NQ / 32; cb += 2) {
+            for (int cb = (warp >> 2); cb < G::NQ / 32; cb += NCG) {
                 float v[32];
                 umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
                 if (!ok) continue;
@@ -460,6 +496,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
     unsigned char* sA = sm;
     unsigned char* sH = sm + G::A_BYTES;
     unsigned char* sW = sH + G::H_BYTES;           // 2 x (W1_j | W2_j)
+    const uint32_t sA_u32 = umma::smem_u32(sA), sH_u32 = umma::smem_u32(sH);
     __shared__ uint64_t bar_w[2], bar_m1, bar_m2;
     __shared__ uint32_t tmem_slot;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -510,7 +547,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
             for (int u = 0; u < RB; ++u) {
                 const int r = warp + (rb + u) * (LP_THREADS / 32);
                 const long long gi = tile * TM + r;
-                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA, r, lane);
+                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
                 if (a.ln2_style == 1 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
             }
         }
@@ -538,11 +575,11 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
             umma::mbar_wait(&bar_m1, ph1);
             ph1 ^= 1;
             umma::fence_after_sync();
-            // ---- epilogue 1: H_j = bf16(gelu(acc1 + b1_j)), 64 columns per warp -------------------
+            // ---- epilogue 1: H_j = bf16(gelu(acc1 + b1_j)), 32 columns per warp -------------------
             {
                 const int r = (warp & 3) * 32 + lane;
 #pragma unroll 1
-                for (int cb = (warp >> 2) * 2; cb < (warp >> 2) * 2 + 2; ++cb) {
+                for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG) {
                     float v[32];
                     umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
                     const float* b1 = a.bias + j * G::HC + cb * 32;
@@ -551,11 +588,10 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
                         uint32_t p[4];
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
-                            p[e] = pack_bf16(gelu_erf(v[c * 8 + 2 * e] + __ldg(b1 + c * 8 + 2 * e)),
-                                             gelu_erf(v[c * 8 + 2 * e + 1] + __ldg(b1 + c * 8 + 2 * e + 1)));
+                            p[e] = pack_bf16(gelu_fast(v[c * 8 + 2 * e] + __ldg(b1 + c * 8 + 2 * e)),
+                                             gelu_fast(v[c * 8 + 2 * e + 1] + __ldg(b1 + c * 8 + 2 * e + 1)));
                         const int col = cb * 32 + c * 8;          // hidden column inside the chunk = K of GEMM 2
-                        *reinterpret_cast<uint4*>(sH + (col >> 6) * (TM * 128) + umma::sw128_chunk(r, (col & 63) >> 3)) =
-                            make_uint4(p[0], p[1], p[2], p[3]);
+                        sts128(sH_u32 + (col >> 6) * (TM * 128) + umma::sw128_chunk(r, (col & 63) >> 3), p[0], p[1], p[2], p[3]);
                     }
                 }
             }
@@ -581,7 +617,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
         {
             const int r = (warp & 3) * 32 + lane;
             const long long gi = tile * TM + r;
-            for (int cb = (warp >> 2); cb < D / 32; cb += 2) {
+            for (int cb = (warp >> 2); cb < D / 32; cb += NCG) {
                 float v[32];
                 umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + G::HC + cb * 32, v);
                 if (gi < a.M) {
