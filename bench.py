@@ -40,6 +40,10 @@ def parse():
     return p.parse_args()
 
 
+# DRAM bytes of the fv_sample launch from the committed ncu capture (profiles/), keyed by (workload, batch)
+NCU_TRAFFIC = {("cfg5", 1024): 837.4e9}
+
+
 def algorithmic_kv_bytes_per_sample(w, rowptr):
     """KV rows named by the mask only: read sum_t nnz(t) rows + write N rows,
     each 2d bf16 = 4d bytes, per layer."""
@@ -152,6 +156,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2606_22984_b200 import binding as fv
     from paper_2606_22984_b200 import build as fvbuild
+    from paper_2606_22984_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -220,10 +225,8 @@ def run_ours(args):
     t_sample = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     t_logp = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
     t_rest = sum(e[2].elapsed_time(e[3]) for e in evs) / args.steps
-    if world > 1:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = shard.max_over_ranks(total_ms, device="cuda")          # multi-GPU time = max over ranks
+    Fq_mean, Fq_std = shard.merge_free_energy(shard.local_moments(E, logq_tf, T))   # the one data exchange
     ms_per_step = total_ms / args.steps
     value = world * B / (ms_per_step * 1e-3)
 
@@ -251,10 +254,7 @@ def run_ours(args):
     eb.record()
     sync_all()
     e2e_ms = ea.elapsed_time(eb)
-    if world > 1:
-        tt = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
+    e2e_ms = shard.max_over_ranks(e2e_ms, device="cuda")
     e2e_value = world * B / (e2e_ms / args.steps * 1e-3)
     h2d = u_host.numel() * 4
     d2h = spins_host.numel() + 4 * B + 4 * B + 16
@@ -272,11 +272,16 @@ def run_ours(args):
             "config": config_of(w, B, world),
             "phases_ms": {"fv_sample": t_sample, "fv_log_prob": t_logp, "energy+free_energy": t_rest},
             "us_per_site_step": 1e3 * t_sample / N,
-            "F_q": {"mean": float(F_val[0]), "std": float(F_val[1]), "per_spin": float(F_val[0]) / N},
-            "roofline": {"kernel": "fv_forward_kernel (SAMPLE mode = fv_sample)", "bound": "hbm",
+            "F_q": {"mean": Fq_mean, "std": Fq_std, "per_spin": Fq_mean / N,
+                    "rank0_kernel": [float(F_val[0]), float(F_val[1])]},
+            "roofline": {"kernel": "fv_decode_kernel (fv_sample: persistent KV-ring sampler)", "bound": "hbm",
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": (rd + wr) * B, "traffic": None},
+                         "algorithmic_bytes_per_launch": (rd + wr) * B,
+                         "traffic": NCU_TRAFFIC.get((w.name, B)),
+                         "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
+                                           "capture of this launch (profiles/r01_fv_sample_ring.md); null for "
+                                           "workloads that were not captured"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches), "clocks": clocks,
         }

@@ -135,7 +135,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn; };
     const bool lp_tc = !cfg->has_wo && (d == 32 || d == 64 || d == 128);   // fv_logprob.cu path
     const int KP = d < 64 ? 64 : d;
-    std::vector<uint16_t> img((size_t)std::max(3 * d * KP, (f / 128) * (128 * KP + d * 128)));
+    const int HC = FV_LP_HC;
+    std::vector<uint16_t> img((size_t)std::max(3 * d * KP, (f / HC) * (HC * KP + d * HC)));
     std::vector<Off> off(NL);
     const float* w = weights;
     const size_t o_tok = A.put(w, sizeof(float) * 2 * cfg->d_token);
@@ -167,15 +168,15 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         o.ln2g = A.put(w, 4 * d); w += d;
         o.ln2b = A.put(w, 4 * d); w += d;
         pack_mma_a(w, f, d, pk.data());
-        if (lp_tc) {                                  // per 128-column hidden chunk: W1_j | W2_j
+        if (lp_tc) {                                  // per HC-column hidden chunk: W1_j | W2_j
             const float* W1 = w;
             const float* W2 = w + (size_t)f * d + f;   // after W1 and b1
-            const size_t per = (size_t)128 * KP + (size_t)d * 128;
-            for (int j = 0; j < f / 128; ++j) {
-                fv_pack_sw128(W1 + (size_t)j * 128 * d, 128, d, d, KP, img.data() + j * per);
-                fv_pack_sw128(W2 + (size_t)j * 128, d, 128, f, 128, img.data() + j * per + (size_t)128 * KP);
+            const size_t per = (size_t)HC * KP + (size_t)d * HC;
+            for (int j = 0; j < f / HC; ++j) {
+                fv_pack_sw128(W1 + (size_t)j * HC * d, HC, d, d, KP, img.data() + j * per);
+                fv_pack_sw128(W2 + (size_t)j * HC, d, HC, f, HC, img.data() + j * per + (size_t)HC * KP);
             }
-            o.img_ffn = A.put(img.data(), (size_t)(f / 128) * per * 2);
+            o.img_ffn = A.put(img.data(), (size_t)(f / HC) * per * 2);
         }
         w += (size_t)f * d;
         o.w1 = A.put(pk.data(), (size_t)f * d * 2);

@@ -6,6 +6,9 @@
 
 #define FV_MAX_LAYERS 16
 
+// Hidden columns per chunk of the fused FFN of fv_logprob.cu (host image packer and kernel must agree).
+constexpr int FV_LP_HC = 64;
+
 // KV rows per ring chunk of the decode kernel (host plan and device kernel must agree).
 #ifndef FV_DEC_CH128
 #define FV_DEC_CH128 16

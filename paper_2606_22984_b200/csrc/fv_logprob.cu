@@ -22,6 +22,8 @@ using namespace fvdev;
 
 constexpr int LP_THREADS = 512;   // 16 warps: warp w reads TMEM lanes 32 (w % 4) .. +31, column group w / 4
 constexpr int NCG = LP_THREADS / 128;   // column groups sharing one TMEM lane quarter
+constexpr int FFN_THREADS = 256;  // the FFN kernel runs 2 CTAs per SM (one normalises/stores while the other is in GELU)
+constexpr int NCG_F = FFN_THREADS / 128;
 constexpr int TM = 128;           // rows per tile = UMMA M
 
 template <int D> struct LpGeo {
@@ -34,13 +36,13 @@ template <int D> struct LpGeo {
     static constexpr int QKV_SMEM = 1024 + A_BYTES + WQ_BYTES + 64;
     static constexpr int TMEM_Q = NQ <= 128 ? 128 : (NQ <= 256 ? 256 : 512);
     // FFN: hidden 4d in chunks of HC columns
-    static constexpr int HC = 128;
+    static constexpr int HC = FV_LP_HC;
     static constexpr int NHC = 4 * D / HC;
     static constexpr int W1_BYTES = HC * KP * 2;          // [HC rows x KP]
     static constexpr int W2_BYTES = D * HC * 2;           // [D rows x HC]
     static constexpr int H_BYTES = TM * HC * 2;
     static constexpr int WBUF = W1_BYTES + W2_BYTES;
-    static constexpr int FFN_SMEM = 1024 + A_BYTES + H_BYTES + 2 * WBUF + 64;
+    static constexpr int FFN_SMEM = A_BYTES + H_BYTES + 2 * WBUF;
     static constexpr int TMEM_F = (HC + D) <= 256 ? 256 : 512;
 };
 
@@ -483,16 +485,17 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
 
 // --------------------------------------------------------------------------------- FFN
 // h <- h + W2 gelu(W1 LN2(h) + b1) + b2 for a tile of 128 rows (Alg. 2 l.16 form; ln2_style 1:
-// h <- LN2(h) first, Alg. 1 l.5).  The hidden layer is processed in chunks of HC = 128 columns:
-//   acc1 (TMEM cols [0,128))  = A W1_j^T         8 (K = 16) MMAs
+// h <- LN2(h) first, Alg. 1 l.5).  The hidden layer is processed in chunks of HC columns:
+//   acc1 (TMEM cols [0,HC))   = A W1_j^T
 //   H_j = bf16(gelu(acc1 + b1_j)) -> shared memory, swizzled K-major (it is GEMM 2's A operand)
-//   acc2 (TMEM cols [128,128+D)) += H_j W2_j^T
+//   acc2 (TMEM cols [HC,HC+D)) += H_j W2_j^T
 // W1_j | W2_j arrive as pre-swizzled images by cp.async.bulk, double buffered.
 template <int D>
-__global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_constant__ LpArgs a) {
+__global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_constant__ LpArgs a) {
     using G = LpGeo<D>;
-    extern __shared__ unsigned char lp_raw[];
-    unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(lp_raw) + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) unsigned char lp_raw_ffn[];   // no alignment slack: two CTAs share an SM
+    unsigned char* sm = lp_raw_ffn;
+    if (umma::smem_u32(sm) & 1023u) __trap();
     unsigned char* sA = sm;
     unsigned char* sH = sm + G::A_BYTES;
     unsigned char* sW = sH + G::H_BYTES;           // 2 x (W1_j | W2_j)
@@ -506,7 +509,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
         umma::fence_mbar_init();
     }
     if (warp == 0) umma::tmem_alloc<G::TMEM_F>(&tmem_slot);
-    if (D < 64) for (int i = tid; i < G::A_BYTES / 16; i += LP_THREADS) reinterpret_cast<uint4*>(sA)[i] = make_uint4(0, 0, 0, 0);
+    if (D < 64) for (int i = tid; i < G::A_BYTES / 16; i += FFN_THREADS) reinterpret_cast<uint4*>(sA)[i] = make_uint4(0, 0, 0, 0);
     umma::fence_before_sync();
     __syncthreads();
     umma::fence_after_sync();
@@ -528,15 +531,26 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
         }
     };
     if (tid == 0 && n_chunks > 0) issue_w(0);
-    uint32_t ph1 = 0, ph2 = 0;
+    auto issue_mma1 = [&](unsigned char* w1) {               // thread 0: acc1 = A W1_j^T
+        const uint32_t a0 = umma::smem_u32(sA), b0 = umma::smem_u32(w1);
+#pragma unroll
+        for (int kb = 0; kb < G::KB; ++kb)
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+                umma::mma_bf16_ss(tmem, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
+                                  umma::make_desc_sw128(b0 + kb * (G::HC * 128) + ks * 32), idesc1, (kb | ks) != 0);
+        umma::commit(&bar_m1);
+    };
+    uint32_t ph1 = 0;
+    long long n_m2 = 0;                                      // GEMM 2 commits so far (parity of bar_m2)
     long long gch = 0;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         // ---- prologue: LN2 -> bf16 A tile (ln2_style 1: the residual stream becomes LN2(h)) -----
-        for (int rb = 0; rb < TM / (LP_THREADS / 32); rb += RB) {
+        for (int rb = 0; rb < TM / (FFN_THREADS / 32); rb += RB) {
             float x[RB][E];
 #pragma unroll
             for (int u = 0; u < RB; ++u) {
-                const long long gi = tile * TM + warp + (rb + u) * (LP_THREADS / 32);
+                const long long gi = tile * TM + warp + (rb + u) * (FFN_THREADS / 32);
                 if (gi < a.M) ld_row<E>(a.h + gi * D + lane * E, x[u]);
                 else {
 #pragma unroll
@@ -545,7 +559,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
             }
 #pragma unroll
             for (int u = 0; u < RB; ++u) {
-                const int r = warp + (rb + u) * (LP_THREADS / 32);
+                const int r = warp + (rb + u) * (FFN_THREADS / 32);
                 const long long gi = tile * TM + r;
                 ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
                 if (a.ln2_style == 1 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
@@ -553,33 +567,24 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
         }
         umma::fence_smem_to_async();
         __syncthreads();
+        if (tid == 0) {                                // GEMM 1 of the tile's first chunk
+            umma::mbar_wait(&bar_w[gch & 1], (uint32_t)((gch >> 1) & 1));
+            umma::fence_after_sync();
+            issue_mma1(sW + (gch & 1) * G::WBUF);
+        }
         for (int j = 0; j < G::NHC; ++j, ++gch) {
-            const int buf = (int)(gch & 1);
-            unsigned char* w1 = sW + buf * G::WBUF;
-            unsigned char* w2 = w1 + G::W1_BYTES;
-            if (tid == 0) {
-                umma::mbar_wait(&bar_w[buf], (uint32_t)((gch >> 1) & 1));
-                umma::fence_after_sync();
-                const uint32_t a0 = umma::smem_u32(sA), b0 = umma::smem_u32(w1);
-#pragma unroll
-                for (int kb = 0; kb < G::KB; ++kb)
-#pragma unroll
-                    for (int ks = 0; ks < 4; ++ks)
-                        umma::mma_bf16_ss(tmem, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
-                                          umma::make_desc_sw128(b0 + kb * (G::HC * 128) + ks * 32), idesc1, (kb | ks) != 0);
-                umma::commit(&bar_m1);
-            }
-            // the previous chunk's GEMM 2 must be done before H (and its weight buffer) is reused
-            if (j > 0) { umma::mbar_wait(&bar_m2, ph2); ph2 ^= 1; }   // (j == 0: waited by epilogue 2)
-            if (tid == 0 && gch + 1 < n_chunks) issue_w(gch + 1);
+            unsigned char* w2 = sW + (int)(gch & 1) * G::WBUF + G::W1_BYTES;
+            // GEMM 1 of this chunk done; tcgen05 ops of one thread complete in issue order, so the
+            // previous chunk's GEMM 2 is done too: H and the other weight buffer are free
             umma::mbar_wait(&bar_m1, ph1);
             ph1 ^= 1;
             umma::fence_after_sync();
+            if (tid == 0 && gch + 1 < n_chunks) issue_w(gch + 1);
             // ---- epilogue 1: H_j = bf16(gelu(acc1 + b1_j)), 32 columns per warp -------------------
             {
                 const int r = (warp & 3) * 32 + lane;
 #pragma unroll 1
-                for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG) {
+                for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG_F) {
                     float v[32];
                     umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
                     const float* b1 = a.bias + j * G::HC + cb * 32;
@@ -608,16 +613,22 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_ffn_kernel(const __grid_cons
                         umma::mma_bf16_ss(tmem + G::HC, umma::make_desc_sw128(h0 + kb * (TM * 128) + ks * 32),
                                           umma::make_desc_sw128(b0 + kb * (D * 128) + ks * 32), idesc2, (j | kb | ks) != 0);
                 umma::commit(&bar_m2);
+                if (j + 1 < G::NHC) {                  // next chunk's GEMM 1 right behind: its latency hides
+                    const long long g1 = gch + 1;      // under this chunk's barrier and the next wait
+                    umma::mbar_wait(&bar_w[g1 & 1], (uint32_t)((g1 >> 1) & 1));
+                    umma::fence_after_sync();
+                    issue_mma1(sW + (g1 & 1) * G::WBUF);
+                }
             }
+            ++n_m2;
         }
         // ---- epilogue 2: h += acc2 + b2 -------------------------------------------------------
-        umma::mbar_wait(&bar_m2, ph2);
-        ph2 ^= 1;
+        umma::mbar_wait(&bar_m2, (uint32_t)((n_m2 - 1) & 1));     // the tile's last GEMM 2
         umma::fence_after_sync();
         {
             const int r = (warp & 3) * 32 + lane;
             const long long gi = tile * TM + r;
-            for (int cb = (warp >> 2); cb < D / 32; cb += NCG) {
+            for (int cb = (warp >> 2); cb < D / 32; cb += NCG_F) {
                 float v[32];
                 umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + G::HC + cb * 32, v);
                 if (gi < a.M) {
@@ -697,6 +708,7 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
     const long long n_tiles = (a.M + TM - 1) / TM;
     const int grid = (int)(n_tiles < n_sms ? n_tiles : n_sms);
     const int rows_per_cta = 64;
+    const int grid_ffn = (int)(n_tiles < 2 * n_sms ? n_tiles : 2 * n_sms);
     for (int l = 0; l < m.n_layers; ++l) {
         const FvLayerDev& L = m.layer[l];
         a.layer = l;
@@ -710,7 +722,7 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
                                                                                                 rows_per_cta);
         }
         a.w_img = L.img_ffn; a.bias = L.b1; a.bias2 = L.b2; a.ln_g = L.ln2_g; a.ln_b = L.ln2_b;
-        lp_ffn_kernel<D><<<grid, LP_THREADS, G::FFN_SMEM, s>>>(a);
+        lp_ffn_kernel<D><<<grid_ffn, FFN_THREADS, G::FFN_SMEM, s>>>(a);
     }
     lp_head_kernel<D><<<B, 256, 0, s>>>(a, m.head_wd, m.head_bd, logq, cond_p);
     return cudaGetLastError();
