@@ -169,40 +169,43 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     const long long n_tiles = (a.M + TM - 1) / TM;
     uint32_t ph = 0;
     bool w_ready = false;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        // ---- prologue: (embedding) + LN1 -> bf16 A tile.  A warp owns 16 rows; their loads are
-        //      issued RB rows at a time before any arithmetic (one HBM round trip per batch) ------
-        for (int rb = 0; rb < TM / (LP_THREADS / 32); rb += RB) {
-            float x[RB][E];
+    // A warp owns RB = 8 rows of a tile.  Their loads are issued together, and the NEXT tile's rows are
+    // requested before this tile's epilogue, so the HBM round trip hides under the MMA and the stores.
+    static_assert(TM / (LP_THREADS / 32) == RB, "one load batch per tile");
+    float x[RB][E];
+    auto load_tile = [&](long long tile) {
 #pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const int r = warp + (rb + u) * (LP_THREADS / 32);
-                const long long gi = tile * TM + r;
-                if (gi < a.M) {
-                    if (a.layer == 0) {             // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
-                        const int t = (int)(gi % a.N);
-                        const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
+        for (int u = 0; u < RB; ++u) {
+            const int r = warp + u * (LP_THREADS / 32);
+            const long long gi = tile * TM + r;
+            if (gi < a.M) {
+                if (a.layer == 0) {                 // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
+                    const int t = (int)(gi % a.N);
+                    const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
 #pragma unroll
-                        for (int j = 0; j < E; ++j) {
-                            const int f = lane * E + j;
-                            x[u][j] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
-                                                    : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
-                        }
-                    } else {
-                        ld_row<E>(a.h + gi * D + lane * E, x[u]);
+                    for (int j = 0; j < E; ++j) {
+                        const int f = lane * E + j;
+                        x[u][j] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
+                                                : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
                     }
                 } else {
-#pragma unroll
-                    for (int j = 0; j < E; ++j) x[u][j] = 0.f;
+                    ld_row<E>(a.h + gi * D + lane * E, x[u]);
                 }
-            }
+            } else {
 #pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const int r = warp + (rb + u) * (LP_THREADS / 32);
-                const long long gi = tile * TM + r;
-                if (a.layer == 0 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
-                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
+                for (int j = 0; j < E; ++j) x[u][j] = 0.f;
             }
+        }
+    };
+    if ((long long)blockIdx.x < n_tiles) load_tile(blockIdx.x);
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        // ---- prologue: (embedding) + LN1 -> bf16 A tile ---------------------------------------
+#pragma unroll
+        for (int u = 0; u < RB; ++u) {
+            const int r = warp + u * (LP_THREADS / 32);
+            const long long gi = tile * TM + r;
+            if (a.layer == 0 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
+            ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
         }
         umma::fence_smem_to_async();
         __syncthreads();
@@ -223,6 +226,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
             umma::commit(&bar_mma);
         }
         w_ready = true;
+        if (tile + gridDim.x < n_tiles) load_tile(tile + gridDim.x);
         umma::mbar_wait(&bar_mma, ph);
         ph ^= 1;
         umma::fence_after_sync();
@@ -240,7 +244,10 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
                 if (!ok) continue;
                 const int f0 = cb * 32;
 #pragma unroll
-                for (int j = 0; j < 32; ++j) v[j] += __ldg(a.bias + f0 + j);
+                for (int j = 0; j < 32; j += 4) {
+                    const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias + f0 + j));
+                    v[j] += bb.x; v[j + 1] += bb.y; v[j + 2] += bb.z; v[j + 3] += bb.w;
+                }
                 if (f0 < D) {
 #pragma unroll
                     for (int j = 0; j < 32; j += 4) *reinterpret_cast<float4*>(qrow + f0 + j) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
@@ -587,14 +594,15 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
                 for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG_F) {
                     float v[32];
                     umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
-                    const float* b1 = a.bias + j * G::HC + cb * 32;
+                    const float4* b1 = reinterpret_cast<const float4*>(a.bias + j * G::HC + cb * 32);
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
+                        const float4 ba = __ldg(b1 + 2 * c), bb = __ldg(b1 + 2 * c + 1);
                         uint32_t p[4];
-#pragma unroll
-                        for (int e = 0; e < 4; ++e)
-                            p[e] = pack_bf16(gelu_fast(v[c * 8 + 2 * e] + __ldg(b1 + c * 8 + 2 * e)),
-                                             gelu_fast(v[c * 8 + 2 * e + 1] + __ldg(b1 + c * 8 + 2 * e + 1)));
+                        p[0] = pack_bf16(gelu_fast(v[c * 8 + 0] + ba.x), gelu_fast(v[c * 8 + 1] + ba.y));
+                        p[1] = pack_bf16(gelu_fast(v[c * 8 + 2] + ba.z), gelu_fast(v[c * 8 + 3] + ba.w));
+                        p[2] = pack_bf16(gelu_fast(v[c * 8 + 4] + bb.x), gelu_fast(v[c * 8 + 5] + bb.y));
+                        p[3] = pack_bf16(gelu_fast(v[c * 8 + 6] + bb.z), gelu_fast(v[c * 8 + 7] + bb.w));
                         const int col = cb * 32 + c * 8;          // hidden column inside the chunk = K of GEMM 2
                         sts128(sH_u32 + (col >> 6) * (TM * 128) + umma::sw128_chunk(r, (col & 63) >> 3), p[0], p[1], p[2], p[3]);
                     }
@@ -636,10 +644,8 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
 #pragma unroll
                     for (int jj = 0; jj < 32; jj += 4) {
                         float4 hv = *reinterpret_cast<float4*>(hp + jj);
-                        hv.x += v[jj] + __ldg(a.bias2 + cb * 32 + jj);
-                        hv.y += v[jj + 1] + __ldg(a.bias2 + cb * 32 + jj + 1);
-                        hv.z += v[jj + 2] + __ldg(a.bias2 + cb * 32 + jj + 2);
-                        hv.w += v[jj + 3] + __ldg(a.bias2 + cb * 32 + jj + 3);
+                        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias2 + cb * 32 + jj));
+                        hv.x += v[jj] + bb.x; hv.y += v[jj + 1] + bb.y; hv.z += v[jj + 2] + bb.z; hv.w += v[jj + 3] + bb.w;
                         *reinterpret_cast<float4*>(hp + jj) = hv;
                     }
                 }
