@@ -331,7 +331,12 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
     int nt, grid;
     sample_geometry(B, m->n_sms, &a.rows_per_group, &nt, &a.n_groups, &grid);
     a.uniforms = uniforms; a.spins_out = spins; a.logq = logq; a.cond_p = cond_p;
-    cudaError_t e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, grid,
+    (void)grid;
+    // FLASHVAN_DECODE=cluster opts into the 2-CTA-cluster FFN split (correct, but measured slower than one
+    // CTA per sample group on every BASELINE config: DESIGN.md 6.1)
+    const char* dm = std::getenv("FLASHVAN_DECODE");
+    const int cluster = dm && std::strcmp(dm, "cluster") == 0 && !m->cfg.has_wo;
+    cudaError_t e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, m->n_sms, cluster,
                                      (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "fv_sample launch");
     g_launches++;

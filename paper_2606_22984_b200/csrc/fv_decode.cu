@@ -44,15 +44,25 @@ constexpr int NWC = 16;                       // compute warps
 constexpr int NTHREADS = NWC * 32 + 32;       // + 1 producer warp
 constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
 
-template <int D, int NT>
+// CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
+template <int D, int NT, bool CL = false>
 struct DecGeo {
     using G = Geo<D, NT>;
+    // cluster mode: FFN over the 2R rows of both CTAs, hidden half (2D columns) per CTA
+    static constexpr int R2 = 2 * G::R, FS2 = 2 * D + 8;
+    static constexpr size_t hid2_bytes = (size_t)R2 * FS2 * 2;
+    static constexpr size_t part2_bytes = (size_t)R2 * G::HS * 4;
+    static constexpr size_t big_bytes = !CL ? G::big_bytes
+                                            : (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes);
+    static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
+    static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
+    static constexpr size_t geo_total = G::total - G::big_bytes + big_bytes + xa_bytes + xp_bytes;
     static constexpr int CH = fv_ring_ch(D);              // KV rows per ring chunk (host plan agrees)
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
-    static constexpr size_t fixed = (G::total + 127) / 128 * 128;
+    static constexpr size_t fixed = (geo_total + 127) / 128 * 128;
     static constexpr int TAB_C = 128, TAB_R = 160;        // per-step copy plan staged in smem (x2: t, t+1)
-    static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers, counters, plans
+    static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
     static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
@@ -108,6 +118,33 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // L2 prefetch of a byte range (no shared memory, no completion tracking).
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(src), "r"(bytes) : "memory");
+}
+// ---- 2-CTA cluster plumbing (distributed shared memory) -------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ uint32_t map_to_peer(uint32_t saddr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_peer128(uint32_t raddr, uint4 v) {
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(raddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_peer(uint32_t raddr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(raddr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!done);
 }
 __device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWC * 32) : "memory"); }
 __device__ __forceinline__ int ld_acquire_s32(const int* p) {
@@ -230,11 +267,12 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     }
 }
 
-template <int D, int DH, int NT>
+template <int D, int DH, int NT, bool CL>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
     using G = Geo<D, NT>;
-    using DG = DecGeo<D, NT>;
+    using DG = DecGeo<D, NT, CL>;
+    constexpr int R2 = DG::R2, FS2 = DG::FS2, NT2 = 2 * NT;
     constexpr int R = G::R, HS = G::HS, AS = G::AS, QS = G::QS, FS = G::FS, KS2 = G::KS2;
     constexpr int NSPLIT = (NWC / R) > 1 ? (NWC / R) : 1;    // warps cooperating on one query row
     constexpr int LPR = D / 8, LPH = DH / 8;
@@ -249,16 +287,20 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     unsigned char* big = smem + G::h_bytes + G::a_bytes;
     float* sh_qkv = reinterpret_cast<float*>(big);
     __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
-    float* sh_part = reinterpret_cast<float*>(big + G::hid_bytes);
-    float* sh_split = reinterpret_cast<float*>(big + G::big_bytes);
-    double* sh_logq = reinterpret_cast<double*>(big + G::big_bytes + G::split_bytes);
+    float* sh_part = reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
+    float* sh_split = reinterpret_cast<float*>(big + DG::big_bytes);
+    double* sh_logq = reinterpret_cast<double*>(big + DG::big_bytes + G::split_bytes);
     float* sh_logp = reinterpret_cast<float*>(sh_logq + R);
     float* sh_u = sh_logp + R;
     int* sh_tok = reinterpret_cast<int*>(sh_u + R);
+    // cluster exchange buffers sit at the end of the fixed region (the peer CTA writes them)
+    __nv_bfloat16* sh_a2 = reinterpret_cast<__nv_bfloat16*>(smem + DG::fixed - DG::xa_bytes - DG::xp_bytes);
+    float* sh_xp = reinterpret_cast<float*>(smem + DG::fixed - DG::xp_bytes);
     uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + DG::fixed);
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
     int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
+    uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 2);     // [2] cluster exchange barriers (LN2 rows, partials)
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
     int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
     unsigned char* ring = smem + DG::fixed + DG::bar_bytes;
@@ -270,9 +312,15 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
         *sh_app = 0;
         *sh_issued = 0;
+        if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
+    const uint32_t crank = CL ? cluster_ctarank() : 0;
+    if (CL) cluster_sync_all();                     // the peer's barriers exist before anyone arrives on them
+    // work units: a CTA (a cluster in CL mode) walks sample groups; both CTAs of a cluster iterate alike
+    const int n_walk = CL ? gridDim.x / 2 : gridDim.x, walk0 = CL ? blockIdx.x / 2 : blockIdx.x;
+    const int n_units = CL ? (a.n_groups + 1) / 2 : a.n_groups;
 
     // =============================== PRODUCER WARP ===============================
     // Lanes work on VW consecutive chunks of the ring at once (one chunk per lane: wait for the
@@ -283,8 +331,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         uint32_t seq = 0;
         int it = 0;
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
-        auto issue_weights = [&](const uint4* w, int n) {
-            const unsigned char* src = reinterpret_cast<const unsigned char*>(w);
+        auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
+            const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
             for (int i0 = 0; i0 < n; i0 += VW) {
                 const int i = i0 + lane;
                 if (lane < VW && i < n) {
@@ -292,7 +340,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
                     mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
                     mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
-                    bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * DG::CHUNK_BYTES,
+                    bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
                              (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
                 }
                 __syncwarp();
@@ -300,9 +348,10 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
             }
             seq += (uint32_t)n;
         };
-        for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
-            const int b_first = unit * a.rows_per_group;
-            const int n_own = min(a.rows_per_group, a.B - b_first);
+        for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
+            const int unit = CL ? wu * 2 + (int)crank : wu;
+            const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
+            const int n_own = unit < a.n_groups ? min(a.rows_per_group, a.B - b_first) : 0;   // 0: FFN helper only
             // copy plan of a step: chunk -> run list (staged in shared memory when it fits)
             struct Plan { int nch, nn, nruns; const int32_t* cptr; const int2* rptr; };
             auto stage_plan = [&](int t) {
@@ -391,13 +440,19 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     seq += (uint32_t)total;
                     if (DG::WRING) {
                         if (m.has_wo) issue_weights(L.wo, DG::NO);
-                        issue_weights(L.w1, DG::N1);
-                        issue_weights(L.w2, DG::N2);
+                        if (CL) {     // my half of the hidden layer: rows of W1, K-half of every m-tile of W2
+                            issue_weights(L.w1, DG::N1 / 2, (int)crank * (DG::N1 / 2));
+                            issue_weights(L.w2, DG::N2 / 2, (int)crank, 2);
+                        } else {
+                            issue_weights(L.w1, DG::N1);
+                            issue_weights(L.w2, DG::N2);
+                        }
                     }
                 }
                 cur = nxt;
             }
         }
+        if (CL) cluster_sync_all();                 // matches the compute warps' final cluster barrier
         return;
     }
 
@@ -407,9 +462,10 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint32_t seq_base = 0;
     int it = 0;
     const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
-    for (int unit = blockIdx.x; unit < a.n_groups; unit += gridDim.x, ++it) {
-        const int b_first = unit * a.rows_per_group;
-        const int n_own = min(a.rows_per_group, a.B - b_first);
+    for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
+        const int unit = CL ? wu * 2 + (int)crank : wu;
+        const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
+        const int n_own = unit < a.n_groups ? min(a.rows_per_group, a.B - b_first) : 0;       // 0: FFN helper only
         if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
         for (int t = 0; t < N; ++t) {
             const int me0 = __ldg(m.mask_rowptr + t);
@@ -576,60 +632,135 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                     cbar();
                 }
-                // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
-                for (int r = warp; r < R; r += NWC)
-                    ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
-                cbar();
-                // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
-                {
-                    auto epi = [&](int mt, int, float (&acc)[NT][4]) {
-                        const int f = mt * 16 + g;
-                        const float b0 = __ldg(L.b1 + f), b1 = __ldg(L.b1 + f + 8);
-#pragma unroll
-                        for (int nt = 0; nt < NT; ++nt) {
-                            __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS + f;
-                            o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
-                            o[FS] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
-                            o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
-                            o[FS + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
-                        }
-                    };
-                    if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
-                        seq_base += DG::N1;
-                    } else {
-                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
+                if constexpr (CL) {
+                    // ======== FFN split over the 2-CTA cluster =====================================
+                    // Each CTA streams only HALF of W1/W2 (its 2D hidden columns) and applies them to
+                    // the rows of BOTH CTAs; the halves meet again as two partial sums.
+                    const uint32_t peer = crank ^ 1u;
+                    const uint32_t xpar = (uint32_t)((((long long)it * N + t) * NL + l) & 1);
+                    // ---- LN2 of my rows -> my slot of sh_a2, copy to the peer's sh_a2 -------------
+                    for (int r = warp; r < R; r += NWC)
+                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1,
+                                  sh_a2 + (crank * R + r) * AS, lane);
+                    cbar();
+                    {
+                        constexpr int PCS = R * AS * 2 / 16;            // 16-byte pieces of my R rows
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(sh_a2 + crank * R * AS);
+                        const uint32_t dst = map_to_peer(smem_u32(src), peer);
+                        for (int i = tid; i < PCS; i += NWC * 32)
+                            st_peer128(dst + i * 16, *reinterpret_cast<const uint4*>(src + i * 16));
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_peer(map_to_peer(smem_u32(bar_x), peer));
                     }
-                }
-                cbar();
-                // ---- FFN down-projection, K split KS2 ways into partial buffers -------------
-                {
-                    auto epi = [&](int mt, int ks, float (&acc)[NT][4]) {
-                        const int f = mt * 16 + g;
+                    mbar_wait_cluster(bar_x, xpar);
+                    // ---- FFN1 half + GELU over 2R rows -> bf16 hidden half ------------------------
+                    {
+                        auto epi = [&](int mt, int, float (&acc)[NT2][4]) {
+                            const int f = mt * 16 + g;
+                            const float b0 = __ldg(L.b1 + crank * 2 * D + f), b1 = __ldg(L.b1 + crank * 2 * D + f + 8);
 #pragma unroll
-                        for (int nt = 0; nt < NT; ++nt) {
-                            float* o = sh_part + ((size_t)ks * R + nt * 8 + 2 * c4) * HS + f;
-                            o[0] = acc[nt][0]; o[HS] = acc[nt][1];
-                            o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
-                        }
-                    };
-                    if constexpr (DG::WRING) {
-                        gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
-                        seq_base += DG::N2;
-                    } else {
-                        gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
+                            for (int nt = 0; nt < NT2; ++nt) {
+                                __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS2 + f;
+                                o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
+                                o[FS2] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
+                                o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
+                                o[FS2 + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
+                            }
+                        };
+                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
+                        seq_base += DG::N1 / 2;
                     }
-                }
-                cbar();
-                // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
-                for (int i = tid; i < R * D; i += NWC * 32) {
-                    const int r = i / D, f = i - r * D;
-                    float v = __ldg(L.b2 + f);
+                    cbar();
+                    // ---- FFN2 over my K-half: partial sums for all 2R rows -------------------------
+                    {
+                        auto epi = [&](int mt, int, float (&acc)[NT2][4]) {
+                            const int f = mt * 16 + g;
 #pragma unroll
-                    for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
-                    sh_h[r * HS + f] += v;
+                            for (int nt = 0; nt < NT2; ++nt) {
+                                float* o = sh_part + (nt * 8 + 2 * c4) * HS + f;
+                                o[0] = acc[nt][0]; o[HS] = acc[nt][1];
+                                o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
+                            }
+                        };
+                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
+                        seq_base += DG::N2 / 2;
+                    }
+                    cbar();
+                    {   // the peer's rows of my partial sums -> the peer's sh_xp
+                        constexpr int PCS = R * HS * 4 / 16;
+                        const unsigned char* src = reinterpret_cast<const unsigned char*>(sh_part + peer * R * HS);
+                        const uint32_t dst = map_to_peer(smem_u32(sh_xp), peer);
+                        for (int i = tid; i < PCS; i += NWC * 32)
+                            st_peer128(dst + i * 16, *reinterpret_cast<const uint4*>(src + i * 16));
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_peer(map_to_peer(smem_u32(bar_x + 1), peer));
+                    }
+                    mbar_wait_cluster(bar_x + 1, xpar);
+                    // ---- feed-forward residual; the two halves are added in cluster-rank order ----
+                    for (int i = tid; i < R * D; i += NWC * 32) {
+                        const int r = i / D, f = i - r * D;
+                        const float mine = sh_part[(crank * R + r) * HS + f], theirs = sh_xp[r * HS + f];
+                        const float p0 = crank == 0 ? mine : theirs, p1 = crank == 0 ? theirs : mine;
+                        sh_h[r * HS + f] += (p0 + p1) + __ldg(L.b2 + f);
+                    }
+                    cbar();
+                } else {
+                    // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
+                    for (int r = warp; r < R; r += NWC)
+                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                    cbar();
+                    // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
+                    {
+                        auto epi = [&](int mt, int, float (&acc)[NT][4]) {
+                            const int f = mt * 16 + g;
+                            const float b0 = __ldg(L.b1 + f), b1 = __ldg(L.b1 + f + 8);
+    #pragma unroll
+                            for (int nt = 0; nt < NT; ++nt) {
+                                __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS + f;
+                                o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
+                                o[FS] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
+                                o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
+                                o[FS + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
+                            }
+                        };
+                        if constexpr (DG::WRING) {
+                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
+                            seq_base += DG::N1;
+                        } else {
+                            gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
+                        }
+                    }
+                    cbar();
+                    // ---- FFN down-projection, K split KS2 ways into partial buffers -------------
+                    {
+                        auto epi = [&](int mt, int ks, float (&acc)[NT][4]) {
+                            const int f = mt * 16 + g;
+    #pragma unroll
+                            for (int nt = 0; nt < NT; ++nt) {
+                                float* o = sh_part + ((size_t)ks * R + nt * 8 + 2 * c4) * HS + f;
+                                o[0] = acc[nt][0]; o[HS] = acc[nt][1];
+                                o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
+                            }
+                        };
+                        if constexpr (DG::WRING) {
+                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
+                            seq_base += DG::N2;
+                        } else {
+                            gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
+                        }
+                    }
+                    cbar();
+                    // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
+                    for (int i = tid; i < R * D; i += NWC * 32) {
+                        const int r = i / D, f = i - r * D;
+                        float v = __ldg(L.b2 + f);
+    #pragma unroll
+                        for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                        sh_h[r * HS + f] += v;
+                    }
+                    cbar();
+
                 }
-                cbar();
             }
             // ---- output head: p(+1) = softmax(z)[1] = sigmoid(z1 - z0) (Alg. 2 l.20-22) -----
             for (int r = warp; r < R; r += NWC) {
@@ -658,15 +789,16 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         }
         cbar();
     }
+    if (CL) cluster_sync_all();                     // no CTA leaves while its peer may still write to it
 }
 
 }  // namespace
 
 // ------------------------------------------------------------------------------ dispatch
-template <int D, int DH, int NT>
-static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int grid, cudaStream_t s) {
-    auto kern = fv_decode_kernel<D, DH, NT>;
-    using DG = DecGeo<D, NT>;
+template <int D, int DH, int NT, bool CL>
+static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
+    auto kern = fv_decode_kernel<D, DH, NT, CL>;
+    using DG = DecGeo<D, NT, CL>;
     const size_t smem = DG::total;
     static bool attr_set = false;                 // per instantiation
     if (!attr_set) {
@@ -674,32 +806,59 @@ static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int g
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    kern<<<grid, NTHREADS, smem, s>>>(m, a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.blockDim = dim3(NTHREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    if (CL) {                                     // one CTA per SM, paired: cluster k walks group pairs k, k + n, ...
+        const int pairs = (a.n_groups + 1) / 2, max_pairs = n_sms / 2;
+        cfg.gridDim = dim3(2 * (pairs < max_pairs ? pairs : max_pairs));
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    } else {
+        cfg.gridDim = dim3(a.n_groups < n_sms ? a.n_groups : n_sms);
+    }
+    return cudaLaunchKernelEx(&cfg, kern, m, a);
 }
 
-template <int D, int DH>
-static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArgs& a, int grid, cudaStream_t s) {
+template <int D, int DH, bool CL>
+static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
     switch (nt) {
-        case 1: return launch_dec<D, DH, 1>(m, a, grid, s);
-        case 2: return launch_dec<D, DH, 2>(m, a, grid, s);
-        case 4: return launch_dec<D, DH, 4>(m, a, grid, s);
+        case 1: return launch_dec<D, DH, 1, CL>(m, a, n_sms, s);
+        case 2: return launch_dec<D, DH, 2, CL>(m, a, n_sms, s);
+        case 4: return launch_dec<D, DH, 4, CL>(m, a, n_sms, s);
         default: return cudaErrorInvalidValue;
     }
 }
 
+// cluster = 1: 2-CTA clusters split the FFN (needs the weight ring: d <= 128, and no W_O variant yet).
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt, const FvForwardArgs& a,
-                             int grid, cudaStream_t s) {
+                             int n_sms, int cluster, cudaStream_t s) {
     const int key = d_model * 1000 + d_head;
+    if (cluster && FV_DEC_WRING && d_model <= 128) {
+        switch (key) {
+#ifndef FV_DEC_ONLY_128_16
+            case 32016: return launch_dec_nt<32, 16, true>(m, nt, a, n_sms, s);
+            case 64016: return launch_dec_nt<64, 16, true>(m, nt, a, n_sms, s);
+            case 64032: return launch_dec_nt<64, 32, true>(m, nt, a, n_sms, s);
+            case 128032: return launch_dec_nt<128, 32, true>(m, nt, a, n_sms, s);
+#endif
+            case 128016: return launch_dec_nt<128, 16, true>(m, nt, a, n_sms, s);
+            default: break;
+        }
+    }
     switch (key) {
 #ifndef FV_DEC_ONLY_128_16
-        case 32016: return launch_dec_nt<32, 16>(m, nt, a, grid, s);
-        case 64016: return launch_dec_nt<64, 16>(m, nt, a, grid, s);
-        case 64032: return launch_dec_nt<64, 32>(m, nt, a, grid, s);
-        case 128032: return launch_dec_nt<128, 32>(m, nt, a, grid, s);
-        case 256064: return launch_dec_nt<256, 64>(m, nt, a, grid, s);
+        case 32016: return launch_dec_nt<32, 16, false>(m, nt, a, n_sms, s);
+        case 64016: return launch_dec_nt<64, 16, false>(m, nt, a, n_sms, s);
+        case 64032: return launch_dec_nt<64, 32, false>(m, nt, a, n_sms, s);
+        case 128032: return launch_dec_nt<128, 32, false>(m, nt, a, n_sms, s);
+        case 256064: return launch_dec_nt<256, 64, false>(m, nt, a, n_sms, s);
 #endif
-        case 128016: return launch_dec_nt<128, 16>(m, nt, a, grid, s);
+        case 128016: return launch_dec_nt<128, 16, false>(m, nt, a, n_sms, s);
         default: return cudaErrorInvalidValue;
     }
 }

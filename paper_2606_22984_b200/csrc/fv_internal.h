@@ -78,7 +78,7 @@ cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int 
                               const FvForwardArgs& a, int grid, cudaStream_t s);
 size_t fv_forward_smem_bytes(int d_model, int nt);
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt,
-                             const FvForwardArgs& a, int grid, cudaStream_t s);
+                             const FvForwardArgs& a, int n_sms, int cluster, cudaStream_t s);
 cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
                                  float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s);
 void fv_pack_sw128(const float* W, int rows, int K, int ld, int KP, uint16_t* dst);

@@ -190,3 +190,14 @@ def test_full_size_sampled_rows(name, n_check):
     assert torch.isfinite(lq_g).all() and torch.isfinite(lq_tf).all()
     assert (lq_g - lq_tf).abs().max().item() <= 2e-4 * max(1.0, lq_g.abs().max().item())
     model.close()
+
+
+def test_cluster_decode_variant(monkeypatch):
+    """FLASHVAN_DECODE=cluster: 2-CTA clusters split the FFN over distributed shared memory; checked
+    against the oracle like the default launch (odd number of sample groups: one CTA only helps)."""
+    w = dataclasses.replace(W.CONFIGS["cfg5"], L=12, n_sites=144, window=12)
+    B = 333
+    model, weights, posemb, rp, col = build(w, B)
+    monkeypatch.setenv("FLASHVAN_DECODE", "cluster")
+    ties, flips = check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B))
+    print(f"cluster decode: near-tie sites {ties}, flips among them {flips}")
