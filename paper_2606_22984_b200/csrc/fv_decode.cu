@@ -33,6 +33,9 @@
 #ifndef FV_DEC_PREFETCH
 #define FV_DEC_PREFETCH 0   // 1: L2 prefetch of the next phase's KV runs (measured slower: 348 vs 294 ms on cfg5)
 #endif
+#ifndef FV_DEC_FUSED
+#define FV_DEC_FUSED 0      // 1: fused per-row phases (6 instead of 9-10 CTA barriers per layer; measured neutral on cfg5, slower at 32 rows per CTA)
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -267,12 +270,17 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     }
 }
 
-template <int D, int DH, int NT, bool CL>
+// FUSED: the per-row phases are merged (one warp per row keeps the row from one phase to the next):
+//   [attention combine + KV append + LN2], [FFN residual + next layer's LN1], and for the last layer
+//   [residual + head + Bernoulli + log q + next step's embedding + LN1]: 6 CTA barriers per layer
+//   instead of 9-10.  Not combined with W_O or the cluster split.
+template <int D, int DH, int NT, bool CL, bool FUSED>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
     using G = Geo<D, NT>;
     using DG = DecGeo<D, NT, CL>;
     constexpr int R2 = DG::R2, FS2 = DG::FS2, NT2 = 2 * NT;
+    static_assert(!(CL && FUSED), "fused row phases are for the one-CTA-per-group launch");
     constexpr int R = G::R, HS = G::HS, AS = G::AS, QS = G::QS, FS = G::FS, KS2 = G::KS2;
     constexpr int NSPLIT = (NWC / R) > 1 ? (NWC / R) : 1;    // warps cooperating on one query row
     constexpr int LPR = D / 8, LPH = DH / 8;
@@ -462,6 +470,36 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint32_t seq_base = 0;
     int it = 0;
     const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
+    // FUSED row helpers (one warp, row r; lane holds features lane * D/32 + j throughout)
+    auto embed_ln1 = [&](int r, int t) {            // Eq. 15 (l.287-292) for step t, then layer 0's LN1
+        const int dt = m.d_token, tok = sh_tok[r];
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) {
+            const int f = lane * (D / 32) + j;
+            sh_h[r * HS + f] = f < dt ? __ldg(m.tok_emb + tok * dt + f) : __ldg(m.posemb + (size_t)t * (D - dt) + (f - dt));
+        }
+        ln_row<D>(sh_h + r * HS, m.layer[0].ln1_g, m.layer[0].ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+    };
+    auto head_row = [&](int r, int t, int b_first, int n_own) {   // Alg. 2 l.20-25 for one sample
+        const int b = b_first + r;
+        float d = 0.f;
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) d += sh_h[r * HS + lane * (D / 32) + j] * __ldg(m.head_wd + lane * (D / 32) + j);
+        d = warp_sum(d) + m.head_bd;
+        if (lane == 0) {
+            const float u = __ldg(a.uniforms + (size_t)b * N + t);
+            const float p = 1.0f / (1.0f + expf(-d));
+            const int up = u < p;                                  // reading A10 (l.23)
+            a.spins_out[(size_t)b * N + t] = up ? 1 : -1;           // sigma = 2 s - 1 (l.25)
+            sh_tok[r] = up;
+            const float x = up ? -d : d;                           // log p(s) = -softplus(x)
+            sh_logq[r] += (double)(-(fmaxf(x, 0.f) + log1pf(expf(-fabsf(x)))));
+            if (t == N - 1) a.logq[b] = (float)sh_logq[r];
+            if (a.cond_p) a.cond_p[(size_t)b * N + t] = p;
+        }
+        __syncwarp();                                               // sh_tok[r] visible to the embedding below
+        (void)n_own;
+    };
     for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
         const int unit = CL ? wu * 2 + (int)crank : wu;
         const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
@@ -471,6 +509,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
             const int me0 = __ldg(m.mask_rowptr + t);
             const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
             const int nch = (nn + CH - 1) / CH;
+            if constexpr (!FUSED) {
             if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
             cbar();
             // ---- concatenated positional embedding (Eq. 15, l.287-292) -------------------
@@ -481,12 +520,19 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                           : __ldg(m.posemb + (size_t)t * (D - dt) + (f - dt));
             }
             cbar();
+            } else if (t == 0) {                    // later steps: embedded by the previous step's last phase
+                cbar();                             // sh_tok / sh_logq initialised
+                for (int r = warp; r < R; r += NWC) embed_ln1(r, 0);
+                cbar();
+            }
             for (int l = 0; l < NL; ++l) {
                 const FvLayerDev& L = m.layer[l];
                 // ---- LN1 (Alg. 2 l.12) -> bf16 activations ----------------------------------
-                for (int r = warp; r < R; r += NWC)
-                    ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
-                cbar();
+                if constexpr (!FUSED) {
+                    for (int r = warp; r < R; r += NWC)
+                        ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+                    cbar();
+                }
                 // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13) ---------------------------------
                 {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
@@ -507,21 +553,27 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     }
                 }
                 cbar();
-                // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) -------
-                for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
-                    const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
-                    if (r >= n_own) continue;
-                    const float* s = sh_qkv + r * QS + D + ch * 8;
-                    uint4 v;
-                    v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
-                    v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
-                    __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
-                    *reinterpret_cast<uint4*>(dst) = v;
+                // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2).  Row t itself is
+                //      attended from shared memory, so the stores only have to land before step t+1 ----
+                auto append_kv = [&]() {
+                    for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
+                        const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
+                        if (r >= n_own) continue;
+                        const float* s = sh_qkv + r * QS + D + ch * 8;
+                        uint4 v;
+                        v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
+                        v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
+                        __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
+                        *reinterpret_cast<uint4*>(dst) = v;
+                    }
+                    // the producer reads these rows through the async proxy (cp.async.bulk)
+                    asm volatile("fence.proxy.async.global;\n" ::: "memory");
+                };
+                if constexpr (!FUSED) {
+                    append_kv();
+                    cbar();
+                    if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 }
-                // the producer reads these rows through the async proxy (cp.async.bulk)
-                asm volatile("fence.proxy.async.global;\n" ::: "memory");
-                cbar();
-                if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
                 for (int task = warp; task < R * NSPLIT; task += NWC) {
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
@@ -589,7 +641,34 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 seq_base += (uint32_t)(n_own * nch);
                 cbar();
-                if (NSPLIT > 1) {                       // combine the split partials, fixed order
+                if constexpr (FUSED) {
+                    // ---- phase C: combine the split partials of my rows, LN2; everyone appends K|V ----
+                    for (int r = warp; r < R; r += NWC) {
+                        if (NSPLIT > 1 && r < n_own) {
+                            const float* ps = sh_split + r * NSPLIT * SPS;
+#pragma unroll
+                            for (int j = 0; j < D / 32; ++j) {
+                                const int f = lane * (D / 32) + j;
+                                float mx = -1e30f;
+#pragma unroll
+                                for (int s2 = 0; s2 < NSPLIT; ++s2) mx = fmaxf(mx, ps[s2 * SPS + f / 8]);
+                                float num = 0.f, den = 0.f;
+#pragma unroll
+                                for (int s2 = 0; s2 < NSPLIT; ++s2) {
+                                    const float wgt = exp2f(ps[s2 * SPS + f / 8] - mx);
+                                    den += wgt * ps[s2 * SPS + LPR + f / 8];
+                                    num += wgt * ps[s2 * SPS + 2 * LPR + f];
+                                }
+                                sh_h[r * HS + f] += num / den;
+                            }
+                        }
+                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                    }
+                    append_kv();
+                    cbar();
+                    if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
+                }
+                if (!FUSED && NSPLIT > 1) {             // combine the split partials, fixed order
                     for (int i = tid; i < R * D; i += NWC * 32) {
                         const int r = i / D, f = i - r * D;
                         if (r >= n_own) continue;
@@ -611,7 +690,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     cbar();
                 }
                 // ---- optional output projection (bypassed in the paper, l.107) --------------
-                if (m.has_wo) {
+                if (!FUSED && m.has_wo) {
                     {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
@@ -706,9 +785,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     cbar();
                 } else {
                     // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
-                    for (int r = warp; r < R; r += NWC)
-                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
-                    cbar();
+                    if constexpr (!FUSED) {
+                        for (int r = warp; r < R; r += NWC)
+                            ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                        cbar();
+                    }
                     // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
                     {
                         auto epi = [&](int mt, int, float (&acc)[NT][4]) {
@@ -751,18 +832,42 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     }
                     cbar();
                     // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
-                    for (int i = tid; i < R * D; i += NWC * 32) {
-                        const int r = i / D, f = i - r * D;
-                        float v = __ldg(L.b2 + f);
-    #pragma unroll
-                        for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
-                        sh_h[r * HS + f] += v;
+                    if constexpr (!FUSED) {
+                        for (int i = tid; i < R * D; i += NWC * 32) {
+                            const int r = i / D, f = i - r * D;
+                            float v = __ldg(L.b2 + f);
+#pragma unroll
+                            for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                            sh_h[r * HS + f] += v;
+                        }
+                        cbar();
+                    } else {
+                        // ---- phase R: residual of my rows, then what follows for the row: the next layer's
+                        //      LN1, or (last layer) head + draw + log q + next step's embedding + LN1 -----
+                        for (int r = warp; r < R; r += NWC) {
+#pragma unroll
+                            for (int j = 0; j < D / 32; ++j) {
+                                const int f = lane * (D / 32) + j;
+                                float v = __ldg(L.b2 + f);
+#pragma unroll
+                                for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                                sh_h[r * HS + f] += v;
+                            }
+                            if (l + 1 < NL) {
+                                const FvLayerDev& Ln = m.layer[l + 1];
+                                ln_row<D>(sh_h + r * HS, Ln.ln1_g, Ln.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+                            } else {
+                                if (r < n_own) head_row(r, t, b_first, n_own);
+                                if (t + 1 < N) embed_ln1(r, t + 1);
+                            }
+                        }
+                        cbar();
                     }
-                    cbar();
 
                 }
             }
             // ---- output head: p(+1) = softmax(z)[1] = sigmoid(z1 - z0) (Alg. 2 l.20-22) -----
+            if constexpr (!FUSED) {
             for (int r = warp; r < R; r += NWC) {
                 if (r >= n_own) continue;
                 const int b = b_first + r;
@@ -786,6 +891,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 sh_logq[tid] += (double)sh_logp[tid];
                 if (t == N - 1) a.logq[b_first + tid] = (float)sh_logq[tid];
             }
+            }
         }
         cbar();
     }
@@ -795,9 +901,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
 }  // namespace
 
 // ------------------------------------------------------------------------------ dispatch
-template <int D, int DH, int NT, bool CL>
+template <int D, int DH, int NT, bool CL, bool FUSED>
 static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
-    auto kern = fv_decode_kernel<D, DH, NT, CL>;
+    auto kern = fv_decode_kernel<D, DH, NT, CL, FUSED>;
     using DG = DecGeo<D, NT, CL>;
     const size_t smem = DG::total;
     static bool attr_set = false;                 // per instantiation
@@ -826,10 +932,21 @@ static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n
 
 template <int D, int DH, bool CL>
 static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
+    const bool fused = !CL && !m.has_wo && FV_DEC_FUSED;
+    if (fused) {
+        if constexpr (!CL) {
+            switch (nt) {
+                case 1: return launch_dec<D, DH, 1, false, true>(m, a, n_sms, s);
+                case 2: return launch_dec<D, DH, 2, false, true>(m, a, n_sms, s);
+                case 4: return launch_dec<D, DH, 4, false, true>(m, a, n_sms, s);
+                default: return cudaErrorInvalidValue;
+            }
+        }
+    }
     switch (nt) {
-        case 1: return launch_dec<D, DH, 1, CL>(m, a, n_sms, s);
-        case 2: return launch_dec<D, DH, 2, CL>(m, a, n_sms, s);
-        case 4: return launch_dec<D, DH, 4, CL>(m, a, n_sms, s);
+        case 1: return launch_dec<D, DH, 1, CL, false>(m, a, n_sms, s);
+        case 2: return launch_dec<D, DH, 2, CL, false>(m, a, n_sms, s);
+        case 4: return launch_dec<D, DH, 4, CL, false>(m, a, n_sms, s);
         default: return cudaErrorInvalidValue;
     }
 }
