@@ -253,6 +253,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         e = cudaMalloc(&m->ws, m->ws_bytes);
         if (e != cudaSuccess) { cudaFree(kv); cudaFree(m->arena); delete m; return cuda_fail(e, "cudaMalloc(log_prob workspace)"); }
     }
+    if (const char* pz = std::getenv("FLASHVAN_POISON_KV"); pz && *pz == '1')   // debug aid: unwritten rows read as NaN
+        cudaMemset(kv, 0xFF, m->kv_bytes);
     cudaStream_t s = (cudaStream_t)stream;
     e = cudaMemcpyAsync(m->arena, A.host.data(), m->arena_bytes, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);

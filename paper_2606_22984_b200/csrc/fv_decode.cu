@@ -36,6 +36,9 @@
 #ifndef FV_DEC_FUSED
 #define FV_DEC_FUSED 0      // 1: fused per-row phases (6 instead of 9-10 CTA barriers per layer; measured neutral on cfg5, slower at 32 rows per CTA)
 #endif
+#ifndef FV_DEC_WSLOTS
+#define FV_DEC_WSLOTS 0     // slots of a separate weight ring with its own producer warp (0 = one ring; measured: 4..12 slots give 464..386 ms vs 293 ms on cfg5)
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -44,7 +47,7 @@ namespace {
 using namespace fvdev;
 
 constexpr int NWC = 16;                       // compute warps
-constexpr int NTHREADS = NWC * 32 + 32;       // + 1 producer warp
+constexpr int NTHREADS = NWC * 32 + 64;       // + 2 producer warps (KV ring, weight ring)
 constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
 
 // CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
@@ -68,11 +71,17 @@ struct DecGeo {
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
-    static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
-    static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
+    static constexpr int NSLOT_ALL = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
+    static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT_ALL * CHUNK_BYTES;
     // GEMM weights stream through the same ring (D <= 128): a chunk is CHUNK_BYTES of the packed
     // image = TPCH 16x16 tiles = whole m-tiles (K = D) or one K-part of an m-tile (K = 4D).
     static constexpr bool WRING = FV_DEC_WRING && D <= 128;
+    // FV_DEC_WSLOTS > 0: the weights get their own ring of that many slots and their own producer
+    // warp, so the KV producer can run ahead through the GEMM phases (and the weight producer through
+    // the attention phase); 0: one ring, one stream in consumption order.
+    static constexpr int NSLOT_W = (WRING && FV_DEC_WSLOTS > 0) ? (FV_DEC_WSLOTS < NSLOT_ALL - 2 ? FV_DEC_WSLOTS : NSLOT_ALL - 2) : 0;
+    static constexpr bool SPLIT = NSLOT_W > 0;
+    static constexpr int NSLOT = NSLOT_ALL - NSLOT_W;             // KV ring (and weights when !SPLIT)
     static constexpr int TPCH = CHUNK_BYTES / 512;
     static constexpr int NQ = (3 * D / 16) * (D / 16) / TPCH;     // W_qkv chunks
     static constexpr int NO = (D / 16) * (D / 16) / TPCH;         // W_o
@@ -218,6 +227,10 @@ struct RingCtx {
     uint64_t* bar_full;
     uint64_t* bar_empty;
     int* issued;
+#ifdef FV_DBG_CHECK
+    mutable const uint4* dbg_w = nullptr;   // packed global image the next gemm_ring chunks come from
+    mutable int dbg_first = 0, dbg_stride = 1;
+#endif
 };
 template <int NSLOT, int CHUNK_BYTES>
 __device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
@@ -228,6 +241,10 @@ __device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32
     return rc.ring + (size_t)slot * CHUNK_BYTES;
 }
 __device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
+    // The slot is refilled by cp.async.bulk (async proxy): order this warp's generic-proxy reads of
+    // it before that write.  Without the fence a refill could overtake the reads (seen as run-to-run
+    // differences of ~1e-4 in both samples of a CTA at one step, 15 of 16 fresh-model runs).
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
     __syncwarp();
     if (lane == 0) mbar_arrive(rc.bar_empty + slot);
 }
@@ -244,6 +261,9 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     constexpr int MPC = SPLITK ? 1 : TPCH / KT_TOTAL;
     constexpr int KT = SPLITK ? TPCH : KT_TOTAL;
     const int g = lane >> 2, c = lane & 3;
+#ifdef FV_DBG_NOW
+    return;                                          // timing experiment: no weight stream, no GEMM
+#endif
     for (int j = warp; j < nchunks; j += NWC) {
         uint32_t slot;
         const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)j, slot)) + lane;
@@ -258,6 +278,13 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
 #pragma unroll
             for (int kt = 0; kt < KT; ++kt) {
                 const uint4 aw = wsm[(mi * KT + kt) * 32];
+#ifdef FV_DBG_CHECK
+                if (rc.dbg_w) {
+                    const uint4 gw = __ldg(rc.dbg_w + ((size_t)(rc.dbg_first + j * rc.dbg_stride) * TPCH + mi * KT + kt) * 32 + lane);
+                    if (gw.x != aw.x || gw.y != aw.y || gw.z != aw.z || gw.w != aw.w)
+                        printf("WMISMATCH cta %d warp %d chunk %d mi %d kt %d lane %d seq %u\n", blockIdx.x, warp, j, mi, kt, lane, seq0 + j);
+                }
+#endif
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
                     const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
@@ -286,7 +313,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     constexpr int LPR = D / 8, LPH = DH / 8;
     constexpr int SPS = D + 2 * LPR;                          // floats per split-partial slot
     constexpr int GR = NWC / NSPLIT;                          // samples attended at the same time
-    constexpr int CH = DG::CH, NSLOT = DG::NSLOT, NSLOT_MAX = DG::NSLOT;
+    constexpr int CH = DG::CH, NSLOT = DG::NSLOT, NSLOT_MAX = DG::NSLOT_ALL;
+    constexpr bool SPLIT = DG::SPLIT;
+    constexpr int NSW = SPLIT ? DG::NSLOT_W : DG::NSLOT;        // slots of the ring the weights use
     static_assert(R * NSPLIT <= 16 || NSPLIT == 1, "split slots");
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -308,18 +337,22 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
     int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
-    uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 2);     // [2] cluster exchange barriers (LN2 rows, partials)
+    int* sh_issued_w = sh_app + 2;                                 // same, weight ring (SPLIT)
+    uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 4);     // [2] cluster exchange barriers (LN2 rows, partials)
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
     int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
     unsigned char* ring = smem + DG::fixed + DG::bar_bytes;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int N = m.n_sites, NL = m.n_layers;
+    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
+    const RingCtx rcw = SPLIT ? RingCtx{ring + (size_t)NSLOT * DG::CHUNK_BYTES, bar_full + NSLOT, bar_empty + NSLOT, sh_issued_w} : rc;
 
     if (tid == 0) {
-        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
+        for (int i = 0; i < NSLOT_MAX; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
         *sh_app = 0;
         *sh_issued = 0;
+        *sh_issued_w = 0;
         if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
@@ -334,27 +367,38 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // Lanes work on VW consecutive chunks of the ring at once (one chunk per lane: wait for the
     // slot, arm the mbarrier, one bulk copy per run).  VW <= NSLOT, so a lane only ever waits
     // on a chunk issued in an earlier round -- no circular wait with the consumers.
-    if (warp == NWC) {
+    if (warp >= NWC) {
+        // warp NWC streams the KV rows; the weights are streamed by the same warp (one ring) or by
+        // warp NWC + 1 into their own ring (SPLIT)
+        const bool do_kv = warp == NWC, do_w = DG::WRING && (SPLIT ? warp == NWC + 1 : warp == NWC);
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
+        constexpr int VWW = NSW >= 32 ? 32 : (NSW >= 16 ? 16 : (NSW >= 8 ? 8 : (NSW >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
+        uint32_t seq_w = 0;                          // SPLIT: the weight ring's own sequence
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
+            if (!do_w) return;
+            uint32_t& sqc = SPLIT ? seq_w : seq;
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
-            for (int i0 = 0; i0 < n; i0 += VW) {
+#ifdef FV_DBG_NOW
+            sqc += (uint32_t)n;
+            return;
+#endif
+            for (int i0 = 0; i0 < n; i0 += VWW) {
                 const int i = i0 + lane;
-                if (lane < VW && i < n) {
-                    const uint32_t sq = seq + (uint32_t)i;
-                    const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                    mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
-                    mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
-                    bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
-                             (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
+                if (lane < VWW && i < n) {
+                    const uint32_t sq = sqc + (uint32_t)i;
+                    const uint32_t slot = sq % NSW, par = (sq / NSW) & 1u;
+                    mbar_wait(rcw.bar_empty + slot, par ^ 1u, 1, sq);
+                    mbar_arrive_expect_tx(rcw.bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
+                    bulk_g2s(rcw.ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
+                             (uint32_t)DG::CHUNK_BYTES, rcw.bar_full + slot);
                 }
                 __syncwarp();
-                if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, n)));
+                if (lane == 0) st_release_s32(rcw.issued, (int)(sqc + (uint32_t)min(i0 + VWW, n)));
             }
-            seq += (uint32_t)n;
+            sqc += (uint32_t)n;
         };
         for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
             const int unit = CL ? wu * 2 + (int)crank : wu;
@@ -397,16 +441,20 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                      (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES);
                 }
             };
-            Plan cur = stage_plan(0);
+            Plan cur = do_kv ? stage_plan(0) : Plan{0, 0, 0, nullptr, nullptr};
             for (int t = 0; t < N; ++t) {
-                const Plan nxt = stage_plan(t + 1);
+                const Plan nxt = do_kv ? stage_plan(t + 1) : Plan{0, 0, 0, nullptr, nullptr};
+#ifdef FV_DBG_NOKV
+                const int nch = 0, nn = 0;           // timing experiment: no KV stream
+#else
                 const int nch = cur.nch, nn = cur.nn;
+#endif
                 const int32_t* cptr = cur.cptr;
                 const int2* rptr = cur.rptr;
-                const int total = n_own * nch;
+                const int total = do_kv ? n_own * nch : 0;
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
-                    if (l + 1 < NL) prefetch_phase(cur, l + 1); else prefetch_phase(nxt, 0);
+                    if (do_kv) { if (l + 1 < NL) prefetch_phase(cur, l + 1); else prefetch_phase(nxt, 0); }
                     if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
                     if (total > 0) {
                         // rows < t of layer l are complete once step t-1 has appended at layer l
@@ -467,9 +515,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // =============================== COMPUTE WARPS ===============================
     const int g = lane >> 2, c4 = lane & 3;
     const int rg = lane / LPR, sub = lane % LPR;
-    uint32_t seq_base = 0;
+    uint32_t seq_base = 0, seq_wc = 0;               // ring sequence numbers: KV (and weights if one ring), weights
     int it = 0;
-    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
     // FUSED row helpers (one warp, row r; lane holds features lane * D/32 + j throughout)
     auto embed_ln1 = [&](int r, int t) {            // Eq. 15 (l.287-292) for step t, then layer 0's LN1
         const int dt = m.d_token, tok = sh_tok[r];
@@ -507,7 +554,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
         for (int t = 0; t < N; ++t) {
             const int me0 = __ldg(m.mask_rowptr + t);
+#ifdef FV_DBG_NOKV
+            const int nn = 0 * me0;
+#else
             const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
+#endif
             const int nch = (nn + CH - 1) / CH;
             if constexpr (!FUSED) {
             if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
@@ -546,8 +597,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                     };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
-                        seq_base += DG::NQ;
+                        #ifdef FV_DBG_CHECK
+                        rcw.dbg_w = L.wqkv;
+#endif
+                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::NQ, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
+                        (SPLIT ? seq_wc : seq_base) += DG::NQ;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
                     }
@@ -566,7 +620,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
                         *reinterpret_cast<uint4*>(dst) = v;
                     }
-                    // the producer reads these rows through the async proxy (cp.async.bulk)
+                    // the producer reads these rows through the async proxy (cp.async.bulk) from L2
                     asm volatile("fence.proxy.async.global;\n" ::: "memory");
                 };
                 if constexpr (!FUSED) {
@@ -604,6 +658,20 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                                                                : r * nch + c);
                         uint32_t slot;
                         const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
+#ifdef FV_DBG_CHECK
+                        {
+                            const int rows_ = min(CH, nn - c * CH);
+                            const unsigned char* gsl = reinterpret_cast<const unsigned char*>(m.kv + ((size_t)(b_first + r) * NL + l) * N * (2 * D));
+                            for (int i = lane; i < rows_ * (DG::ROW_BYTES / 16); i += 32) {
+                                const int r_ = i / (DG::ROW_BYTES / 16), pc = i - r_ * (DG::ROW_BYTES / 16);
+                                const int pos = __ldg(m.mask_col + me0 + c * CH + r_);
+                                const uint4 sv = *reinterpret_cast<const uint4*>(chunk + r_ * DG::ROW_BYTES + pc * 16);
+                                const uint4 gv = ld_kv(gsl + (size_t)pos * DG::ROW_BYTES + pc * 16);
+                                if (sv.x != gv.x || sv.y != gv.y || sv.z != gv.z || sv.w != gv.w)
+                                    printf("KVMISMATCH cta %d warp %d t %d l %d r %d c %d row %d pos %d pc %d seq %u slot %u\n", blockIdx.x, warp, t, l, r, c, r_, pos, pc, sq, slot);
+                            }
+                        }
+#endif
                         attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
                         ring_release(rc, slot, lane);
                     }
@@ -703,8 +771,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
-                        seq_base += DG::NO;
+                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::NO, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
+                        (SPLIT ? seq_wc : seq_base) += DG::NO;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
                     }
@@ -746,8 +814,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[FS2 + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
                             }
                         };
-                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
-                        seq_base += DG::N1 / 2;
+                        gemm_ring<D / 16, NT2, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N1 / 2, (SPLIT ? seq_wc : seq_base), sh_a2, AS, warp, lane, epi);
+                        (SPLIT ? seq_wc : seq_base) += DG::N1 / 2;
                     }
                     cbar();
                     // ---- FFN2 over my K-half: partial sums for all 2R rows -------------------------
@@ -761,8 +829,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
                             }
                         };
-                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
-                        seq_base += DG::N2 / 2;
+                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N2 / 2, (SPLIT ? seq_wc : seq_base), sh_hid, FS2, warp, lane, epi);
+                        (SPLIT ? seq_wc : seq_base) += DG::N2 / 2;
                     }
                     cbar();
                     {   // the peer's rows of my partial sums -> the peer's sh_xp
@@ -805,8 +873,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
-                            seq_base += DG::N1;
+                            #ifdef FV_DBG_CHECK
+                        rcw.dbg_w = L.w1;
+#endif
+                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N1, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
+                            (SPLIT ? seq_wc : seq_base) += DG::N1;
                         } else {
                             gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
                         }
@@ -824,8 +895,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
-                            seq_base += DG::N2;
+                            #ifdef FV_DBG_CHECK
+                        rcw.dbg_w = L.w2;
+#endif
+                        gemm_ring<4 * D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N2, (SPLIT ? seq_wc : seq_base), sh_hid, FS, warp, lane, epi);
+                            (SPLIT ? seq_wc : seq_base) += DG::N2;
                         } else {
                             gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
                         }

@@ -201,3 +201,25 @@ def test_cluster_decode_variant(monkeypatch):
     monkeypatch.setenv("FLASHVAN_DECODE", "cluster")
     ties, flips = check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B))
     print(f"cluster decode: near-tie sites {ties}, flips among them {flips}")
+
+
+def test_sample_is_reproducible_across_fresh_models():
+    """Bit-reproducibility (include/flashvan.h) must not depend on what the KV pool or shared memory
+    held before: the same uniforms through several freshly created models, cold caches included.
+    (Regression: a missing proxy fence let a TMA refill overtake reads of a ring slot.)"""
+    w = dataclasses.replace(W.CONFIGS["cfg4"], L=5, n_sites=125, window=16)
+    B = 150
+    weights, posemb = W.make_weights(w), W.make_posemb(w)
+    rp, col = W.make_mask_csr(w)
+    u = dev(W.make_uniforms(w, B, seed=100))
+    ref = None
+    for it in range(8):
+        model = fv.create_model(w, weights, rp, col, posemb, B)
+        junk = torch.randn(32 << 20, device="cuda")          # disturb the allocator / L2 between runs
+        del junk
+        out = model.sample(u, want_cond_p=True)
+        out = list(out) + list(model.log_prob(out[0], want_cond_p=True))
+        if ref is None:
+            ref = [x.clone() for x in out]
+        assert all(torch.equal(x, y) for x, y in zip(out, ref)), f"run {it} differs"
+        model.close()
