@@ -66,7 +66,8 @@ typedef struct {
  *       row t lists the key positions A(t), ascending, unique, all <= t, last entry == t
  *       (Eq. 3 l.102 sums j <= t; Eq. S1 l.555 is the banded special case).
  *   posemb [host] [N, d_model - d_token] fp32 (Eq. 15).
- * Allocates the paged bf16 KV pool: max_batch * n_layers * N rows of 2d bf16 (K then V).
+ * Allocates the paged bf16 KV pool: max_batch * n_layers * N rows of 2d bf16 (K then V), and for
+ * d_model <= 128 without W_O the fv_log_prob workspace (two fp32 arrays [max_batch * N, d_model]).
  * Synchronises `stream`.  *out is owned by the library until fv_destroy_model. */
 int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weights,
                     const int32_t* mask_rowptr, const int32_t* mask_col, const float* posemb,
@@ -83,7 +84,9 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
 
 /* Alg. 1: teacher-forced log q(s) of given configurations.
  *   spins [device] [B,N] int8 in (+-1; other values are undefined behaviour).
- *   logq, cond_p as in fv_sample.  Overwrites the model's KV pool. */
+ *   logq, cond_p as in fv_sample.  Overwrites the model's KV pool and workspace: calls on one model
+ *   must be ordered on one stream.  Enqueues 3 * n_layers + 1 kernels (layer-major tensor-core path) or
+ *   one (chunked teacher forcing: d_model = 256 or has_wo). */
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p,
                 void* stream);
 
