@@ -39,6 +39,12 @@
 #ifndef FV_DEC_WSLOTS
 #define FV_DEC_WSLOTS 0     // slots of a separate weight ring with its own producer warp (0 = one ring; measured: 4..12 slots give 464..386 ms vs 293 ms on cfg5)
 #endif
+#ifndef FV_DEC_STAGGER_NS
+#define FV_DEC_STAGGER_NS 0
+#endif
+#ifndef FV_DEC_STAGGER_GROUPS
+#define FV_DEC_STAGGER_GROUPS 2
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -358,6 +364,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     }
     __syncthreads();
     const uint32_t crank = CL ? cluster_ctarank() : 0;
+#if FV_DEC_STAGGER_NS > 0
+    // All CTAs do identical work, so their phases stay aligned: every SM pulls KV rows from HBM at the same
+    // time and weights from L2 at the same time.  A one-off start offset de-phases them.
+    {
+        const unsigned int total_ns = (blockIdx.x % FV_DEC_STAGGER_GROUPS) * FV_DEC_STAGGER_NS;
+        for (unsigned int w = 0; w < total_ns; w += 1000) __nanosleep(1000);
+    }
+#endif
     if (CL) cluster_sync_all();                     // the peer's barriers exist before anyone arrives on them
     // work units: a CTA (a cluster in CL mode) walks sample groups; both CTAs of a cluster iterate alike
     const int n_walk = CL ? gridDim.x / 2 : gridDim.x, walk0 = CL ? blockIdx.x / 2 : blockIdx.x;

@@ -10,7 +10,7 @@
 //                    activation never leaves the SM (TMEM -> registers -> shared memory)
 // and lp_head_kernel: sigmoid head, log p of the given spin, per-sample fp64 sum (Alg. 1 l.8-9).
 // GEMM operands are bf16 with fp32 accumulation; LayerNorm, softmax, residual stream stay fp32 --
-// the same arithmetic as the decode kernel, so both paths agree with the oracle inside one bound.
+// the same arithmetic as the decode kernel, so both paths sit inside the same error bound.
 #include <cstdlib>
 #include <cstring>
 
