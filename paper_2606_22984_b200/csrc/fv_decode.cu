@@ -5,15 +5,17 @@
 // over the rows A(t) of the CSR mask -> (W_O) -> LN2 -> FFN -> residual; then the sigmoid head,
 // the Bernoulli draw from the caller's uniform and the log q update.
 //
-// What is new against fv_forward.cu (still used by fv_log_prob): the KV gather is decoupled from
-// the compute warps.  The mask is static, so every KV row a step will need -- except the row the
-// step itself appends -- is known long before; one PRODUCER warp walks (t, layer, sample) in the
-// consumers' order and streams the rows named by the mask from the bf16 KV pool into a shared
-// memory ring with cp.async.bulk (TMA 1-D bulk copies, runs of consecutive positions merged into
-// one copy), completing on mbarriers.  The 16 COMPUTE warps read K/V from shared memory, so HBM
-// keeps streaming during the GEMM phases instead of idling (profiles/r01: attention phase 51 %
-// of the step, HBM idle in the other 49 %).  Row t itself is taken from the registers/shared
-// memory of the step that produced it (rounded to bf16 exactly as the pool stores it).
+// The streams are decoupled from the compute warps.  The mask is static, so every KV row a step will
+// need -- except the row the step itself appends -- is known long before; one PRODUCER warp walks
+// (t, layer) in the consumers' order and streams ONE ordered sequence of 8 KB chunks into a shared
+// memory ring with cp.async.bulk (TMA 1-D bulk copies) completing on mbarriers: the layer's W_qkv,
+// the KV rows the mask names for every sample (runs of consecutive positions merged into one copy by
+// the host plan), W_o, W_1, W_2.  The 16 COMPUTE warps read K/V and the mma.sync A fragments from
+// shared memory.  Row t itself is attended from the shared memory of the step that produced it
+// (rounded to bf16 exactly as the pool stores it).
+// Optional (FLASHVAN_DECODE=cluster): 2-CTA clusters in which each CTA streams only its half of
+// W_1/W_2 and applies it to the rows of both CTAs, exchanging LN2 rows and partial sums through
+// distributed shared memory (correct, measured slower: DESIGN.md 6.1).
 #include <cstdio>
 #include "fv_device.cuh"
 
@@ -30,21 +32,6 @@
 #ifndef FV_DEC_WRING
 #define FV_DEC_WRING 1      // 1: GEMM weights stream through the shared-memory ring (TMA), 0: LDG from L2
 #endif
-#ifndef FV_DEC_PREFETCH
-#define FV_DEC_PREFETCH 0   // 1: L2 prefetch of the next phase's KV runs (measured slower: 348 vs 294 ms on cfg5)
-#endif
-#ifndef FV_DEC_FUSED
-#define FV_DEC_FUSED 0      // 1: fused per-row phases (6 instead of 9-10 CTA barriers per layer; measured neutral on cfg5, slower at 32 rows per CTA)
-#endif
-#ifndef FV_DEC_WSLOTS
-#define FV_DEC_WSLOTS 0     // slots of a separate weight ring with its own producer warp (0 = one ring; measured: 4..12 slots give 464..386 ms vs 293 ms on cfg5)
-#endif
-#ifndef FV_DEC_STAGGER_NS
-#define FV_DEC_STAGGER_NS 0
-#endif
-#ifndef FV_DEC_STAGGER_GROUPS
-#define FV_DEC_STAGGER_GROUPS 2
-#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -53,7 +40,7 @@ namespace {
 using namespace fvdev;
 
 constexpr int NWC = 16;                       // compute warps
-constexpr int NTHREADS = NWC * 32 + 64;       // + 2 producer warps (KV ring, weight ring)
+constexpr int NTHREADS = NWC * 32 + 32;       // + 1 producer warp
 constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
 
 // CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
@@ -77,17 +64,11 @@ struct DecGeo {
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
-    static constexpr int NSLOT_ALL = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
-    static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT_ALL * CHUNK_BYTES;
+    static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
+    static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
     // GEMM weights stream through the same ring (D <= 128): a chunk is CHUNK_BYTES of the packed
     // image = TPCH 16x16 tiles = whole m-tiles (K = D) or one K-part of an m-tile (K = 4D).
     static constexpr bool WRING = FV_DEC_WRING && D <= 128;
-    // FV_DEC_WSLOTS > 0: the weights get their own ring of that many slots and their own producer
-    // warp, so the KV producer can run ahead through the GEMM phases (and the weight producer through
-    // the attention phase); 0: one ring, one stream in consumption order.
-    static constexpr int NSLOT_W = (WRING && FV_DEC_WSLOTS > 0) ? (FV_DEC_WSLOTS < NSLOT_ALL - 2 ? FV_DEC_WSLOTS : NSLOT_ALL - 2) : 0;
-    static constexpr bool SPLIT = NSLOT_W > 0;
-    static constexpr int NSLOT = NSLOT_ALL - NSLOT_W;             // KV ring (and weights when !SPLIT)
     static constexpr int TPCH = CHUNK_BYTES / 512;
     static constexpr int NQ = (3 * D / 16) * (D / 16) / TPCH;     // W_qkv chunks
     static constexpr int NO = (D / 16) * (D / 16) / TPCH;         // W_o
@@ -132,10 +113,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int wh
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// L2 prefetch of a byte range (no shared memory, no completion tracking).
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(src), "r"(bytes) : "memory");
 }
 // ---- 2-CTA cluster plumbing (distributed shared memory) -------------------------------------
 __device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
@@ -233,10 +210,6 @@ struct RingCtx {
     uint64_t* bar_full;
     uint64_t* bar_empty;
     int* issued;
-#ifdef FV_DBG_CHECK
-    mutable const uint4* dbg_w = nullptr;   // packed global image the next gemm_ring chunks come from
-    mutable int dbg_first = 0, dbg_stride = 1;
-#endif
 };
 template <int NSLOT, int CHUNK_BYTES>
 __device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
@@ -267,9 +240,6 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     constexpr int MPC = SPLITK ? 1 : TPCH / KT_TOTAL;
     constexpr int KT = SPLITK ? TPCH : KT_TOTAL;
     const int g = lane >> 2, c = lane & 3;
-#ifdef FV_DBG_NOW
-    return;                                          // timing experiment: no weight stream, no GEMM
-#endif
     for (int j = warp; j < nchunks; j += NWC) {
         uint32_t slot;
         const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)j, slot)) + lane;
@@ -284,13 +254,6 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
 #pragma unroll
             for (int kt = 0; kt < KT; ++kt) {
                 const uint4 aw = wsm[(mi * KT + kt) * 32];
-#ifdef FV_DBG_CHECK
-                if (rc.dbg_w) {
-                    const uint4 gw = __ldg(rc.dbg_w + ((size_t)(rc.dbg_first + j * rc.dbg_stride) * TPCH + mi * KT + kt) * 32 + lane);
-                    if (gw.x != aw.x || gw.y != aw.y || gw.z != aw.z || gw.w != aw.w)
-                        printf("WMISMATCH cta %d warp %d chunk %d mi %d kt %d lane %d seq %u\n", blockIdx.x, warp, j, mi, kt, lane, seq0 + j);
-                }
-#endif
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
                     const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
@@ -303,25 +266,18 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     }
 }
 
-// FUSED: the per-row phases are merged (one warp per row keeps the row from one phase to the next):
-//   [attention combine + KV append + LN2], [FFN residual + next layer's LN1], and for the last layer
-//   [residual + head + Bernoulli + log q + next step's embedding + LN1]: 6 CTA barriers per layer
-//   instead of 9-10.  Not combined with W_O or the cluster split.
-template <int D, int DH, int NT, bool CL, bool FUSED>
+template <int D, int DH, int NT, bool CL>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
     using G = Geo<D, NT>;
     using DG = DecGeo<D, NT, CL>;
-    constexpr int R2 = DG::R2, FS2 = DG::FS2, NT2 = 2 * NT;
-    static_assert(!(CL && FUSED), "fused row phases are for the one-CTA-per-group launch");
+    [[maybe_unused]] constexpr int R2 = DG::R2, FS2 = DG::FS2, NT2 = 2 * NT;
     constexpr int R = G::R, HS = G::HS, AS = G::AS, QS = G::QS, FS = G::FS, KS2 = G::KS2;
     constexpr int NSPLIT = (NWC / R) > 1 ? (NWC / R) : 1;    // warps cooperating on one query row
     constexpr int LPR = D / 8, LPH = DH / 8;
     constexpr int SPS = D + 2 * LPR;                          // floats per split-partial slot
     constexpr int GR = NWC / NSPLIT;                          // samples attended at the same time
-    constexpr int CH = DG::CH, NSLOT = DG::NSLOT, NSLOT_MAX = DG::NSLOT_ALL;
-    constexpr bool SPLIT = DG::SPLIT;
-    constexpr int NSW = SPLIT ? DG::NSLOT_W : DG::NSLOT;        // slots of the ring the weights use
+    constexpr int CH = DG::CH, NSLOT = DG::NSLOT, NSLOT_MAX = DG::NSLOT;
     static_assert(R * NSPLIT <= 16 || NSPLIT == 1, "split slots");
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -343,35 +299,23 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
     int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
-    int* sh_issued_w = sh_app + 2;                                 // same, weight ring (SPLIT)
-    uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 4);     // [2] cluster exchange barriers (LN2 rows, partials)
+    uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 2);     // [2] cluster exchange barriers (LN2 rows, partials)
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
     int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
     unsigned char* ring = smem + DG::fixed + DG::bar_bytes;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int N = m.n_sites, NL = m.n_layers;
-    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
-    const RingCtx rcw = SPLIT ? RingCtx{ring + (size_t)NSLOT * DG::CHUNK_BYTES, bar_full + NSLOT, bar_empty + NSLOT, sh_issued_w} : rc;
 
     if (tid == 0) {
-        for (int i = 0; i < NSLOT_MAX; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
+        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
         *sh_app = 0;
         *sh_issued = 0;
-        *sh_issued_w = 0;
         if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
     const uint32_t crank = CL ? cluster_ctarank() : 0;
-#if FV_DEC_STAGGER_NS > 0
-    // All CTAs do identical work, so their phases stay aligned: every SM pulls KV rows from HBM at the same
-    // time and weights from L2 at the same time.  A one-off start offset de-phases them.
-    {
-        const unsigned int total_ns = (blockIdx.x % FV_DEC_STAGGER_GROUPS) * FV_DEC_STAGGER_NS;
-        for (unsigned int w = 0; w < total_ns; w += 1000) __nanosleep(1000);
-    }
-#endif
     if (CL) cluster_sync_all();                     // the peer's barriers exist before anyone arrives on them
     // work units: a CTA (a cluster in CL mode) walks sample groups; both CTAs of a cluster iterate alike
     const int n_walk = CL ? gridDim.x / 2 : gridDim.x, walk0 = CL ? blockIdx.x / 2 : blockIdx.x;
@@ -381,38 +325,27 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // Lanes work on VW consecutive chunks of the ring at once (one chunk per lane: wait for the
     // slot, arm the mbarrier, one bulk copy per run).  VW <= NSLOT, so a lane only ever waits
     // on a chunk issued in an earlier round -- no circular wait with the consumers.
-    if (warp >= NWC) {
-        // warp NWC streams the KV rows; the weights are streamed by the same warp (one ring) or by
-        // warp NWC + 1 into their own ring (SPLIT)
-        const bool do_kv = warp == NWC, do_w = DG::WRING && (SPLIT ? warp == NWC + 1 : warp == NWC);
+    if (warp == NWC) {
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
-        constexpr int VWW = NSW >= 32 ? 32 : (NSW >= 16 ? 16 : (NSW >= 8 ? 8 : (NSW >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
-        uint32_t seq_w = 0;                          // SPLIT: the weight ring's own sequence
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
-            if (!do_w) return;
-            uint32_t& sqc = SPLIT ? seq_w : seq;
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
-#ifdef FV_DBG_NOW
-            sqc += (uint32_t)n;
-            return;
-#endif
-            for (int i0 = 0; i0 < n; i0 += VWW) {
+            for (int i0 = 0; i0 < n; i0 += VW) {
                 const int i = i0 + lane;
-                if (lane < VWW && i < n) {
-                    const uint32_t sq = sqc + (uint32_t)i;
-                    const uint32_t slot = sq % NSW, par = (sq / NSW) & 1u;
-                    mbar_wait(rcw.bar_empty + slot, par ^ 1u, 1, sq);
-                    mbar_arrive_expect_tx(rcw.bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
-                    bulk_g2s(rcw.ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
-                             (uint32_t)DG::CHUNK_BYTES, rcw.bar_full + slot);
+                if (lane < VW && i < n) {
+                    const uint32_t sq = seq + (uint32_t)i;
+                    const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                    mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
+                    mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
+                    bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
+                             (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
                 }
                 __syncwarp();
-                if (lane == 0) st_release_s32(rcw.issued, (int)(sqc + (uint32_t)min(i0 + VWW, n)));
+                if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, n)));
             }
-            sqc += (uint32_t)n;
+            seq += (uint32_t)n;
         };
         for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
             const int unit = CL ? wu * 2 + (int)crank : wu;
@@ -441,34 +374,15 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 return p;
             };
-            // HBM -> L2 prefetch of every KV run a later phase will copy: the ring then only has to
-            // cover the L2 -> shared memory latency, not the HBM latency.
-            auto prefetch_phase = [&](const Plan& p, int l) {
-                if (!FV_DEC_PREFETCH || p.nruns == 0 || p.rptr == m.runs) return;
-                const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
-                    m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
-                const int items = n_own * p.nruns;
-                for (int i = lane; i < items; i += 32) {
-                    const int r = i / p.nruns, j = i - r * p.nruns;
-                    const int2 run = p.rptr[j];
-                    bulk_prefetch_l2(src_l + ((size_t)r * NL * N + run.x) * DG::ROW_BYTES,
-                                     (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES);
-                }
-            };
-            Plan cur = do_kv ? stage_plan(0) : Plan{0, 0, 0, nullptr, nullptr};
+            Plan cur = stage_plan(0);
             for (int t = 0; t < N; ++t) {
-                const Plan nxt = do_kv ? stage_plan(t + 1) : Plan{0, 0, 0, nullptr, nullptr};
-#ifdef FV_DBG_NOKV
-                const int nch = 0, nn = 0;           // timing experiment: no KV stream
-#else
+                const Plan nxt = stage_plan(t + 1);
                 const int nch = cur.nch, nn = cur.nn;
-#endif
                 const int32_t* cptr = cur.cptr;
                 const int2* rptr = cur.rptr;
-                const int total = do_kv ? n_own * nch : 0;
+                const int total = n_own * nch;
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
-                    if (do_kv) { if (l + 1 < NL) prefetch_phase(cur, l + 1); else prefetch_phase(nxt, 0); }
                     if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
                     if (total > 0) {
                         // rows < t of layer l are complete once step t-1 has appended at layer l
@@ -529,38 +443,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // =============================== COMPUTE WARPS ===============================
     const int g = lane >> 2, c4 = lane & 3;
     const int rg = lane / LPR, sub = lane % LPR;
-    uint32_t seq_base = 0, seq_wc = 0;               // ring sequence numbers: KV (and weights if one ring), weights
+    uint32_t seq_base = 0;
     int it = 0;
-    // FUSED row helpers (one warp, row r; lane holds features lane * D/32 + j throughout)
-    auto embed_ln1 = [&](int r, int t) {            // Eq. 15 (l.287-292) for step t, then layer 0's LN1
-        const int dt = m.d_token, tok = sh_tok[r];
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) {
-            const int f = lane * (D / 32) + j;
-            sh_h[r * HS + f] = f < dt ? __ldg(m.tok_emb + tok * dt + f) : __ldg(m.posemb + (size_t)t * (D - dt) + (f - dt));
-        }
-        ln_row<D>(sh_h + r * HS, m.layer[0].ln1_g, m.layer[0].ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
-    };
-    auto head_row = [&](int r, int t, int b_first, int n_own) {   // Alg. 2 l.20-25 for one sample
-        const int b = b_first + r;
-        float d = 0.f;
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) d += sh_h[r * HS + lane * (D / 32) + j] * __ldg(m.head_wd + lane * (D / 32) + j);
-        d = warp_sum(d) + m.head_bd;
-        if (lane == 0) {
-            const float u = __ldg(a.uniforms + (size_t)b * N + t);
-            const float p = 1.0f / (1.0f + expf(-d));
-            const int up = u < p;                                  // reading A10 (l.23)
-            a.spins_out[(size_t)b * N + t] = up ? 1 : -1;           // sigma = 2 s - 1 (l.25)
-            sh_tok[r] = up;
-            const float x = up ? -d : d;                           // log p(s) = -softplus(x)
-            sh_logq[r] += (double)(-(fmaxf(x, 0.f) + log1pf(expf(-fabsf(x)))));
-            if (t == N - 1) a.logq[b] = (float)sh_logq[r];
-            if (a.cond_p) a.cond_p[(size_t)b * N + t] = p;
-        }
-        __syncwarp();                                               // sh_tok[r] visible to the embedding below
-        (void)n_own;
-    };
+    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
     for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
         const int unit = CL ? wu * 2 + (int)crank : wu;
         const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
@@ -568,13 +453,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
         for (int t = 0; t < N; ++t) {
             const int me0 = __ldg(m.mask_rowptr + t);
-#ifdef FV_DBG_NOKV
-            const int nn = 0 * me0;
-#else
             const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
-#endif
             const int nch = (nn + CH - 1) / CH;
-            if constexpr (!FUSED) {
             if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
             cbar();
             // ---- concatenated positional embedding (Eq. 15, l.287-292) -------------------
@@ -585,19 +465,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                           : __ldg(m.posemb + (size_t)t * (D - dt) + (f - dt));
             }
             cbar();
-            } else if (t == 0) {                    // later steps: embedded by the previous step's last phase
-                cbar();                             // sh_tok / sh_logq initialised
-                for (int r = warp; r < R; r += NWC) embed_ln1(r, 0);
-                cbar();
-            }
             for (int l = 0; l < NL; ++l) {
                 const FvLayerDev& L = m.layer[l];
                 // ---- LN1 (Alg. 2 l.12) -> bf16 activations ----------------------------------
-                if constexpr (!FUSED) {
-                    for (int r = warp; r < R; r += NWC)
-                        ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
-                    cbar();
-                }
+                for (int r = warp; r < R; r += NWC)
+                    ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+                cbar();
                 // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13) ---------------------------------
                 {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
@@ -611,37 +484,28 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                     };
                     if constexpr (DG::WRING) {
-                        #ifdef FV_DBG_CHECK
-                        rcw.dbg_w = L.wqkv;
-#endif
-                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::NQ, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
-                        (SPLIT ? seq_wc : seq_base) += DG::NQ;
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
+                        seq_base += DG::NQ;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
                     }
                 }
                 cbar();
-                // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2).  Row t itself is
-                //      attended from shared memory, so the stores only have to land before step t+1 ----
-                auto append_kv = [&]() {
-                    for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
-                        const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
-                        if (r >= n_own) continue;
-                        const float* s = sh_qkv + r * QS + D + ch * 8;
-                        uint4 v;
-                        v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
-                        v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
-                        __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
-                        *reinterpret_cast<uint4*>(dst) = v;
-                    }
-                    // the producer reads these rows through the async proxy (cp.async.bulk) from L2
-                    asm volatile("fence.proxy.async.global;\n" ::: "memory");
-                };
-                if constexpr (!FUSED) {
-                    append_kv();
-                    cbar();
-                    if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
+                // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) -------
+                for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
+                    const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
+                    if (r >= n_own) continue;
+                    const float* s = sh_qkv + r * QS + D + ch * 8;
+                    uint4 v;
+                    v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
+                    v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
+                    __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
+                    *reinterpret_cast<uint4*>(dst) = v;
                 }
+                // the producer reads these rows through the async proxy (cp.async.bulk)
+                asm volatile("fence.proxy.async.global;\n" ::: "memory");
+                cbar();
+                if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
                 for (int task = warp; task < R * NSPLIT; task += NWC) {
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
@@ -672,20 +536,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                                                                : r * nch + c);
                         uint32_t slot;
                         const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
-#ifdef FV_DBG_CHECK
-                        {
-                            const int rows_ = min(CH, nn - c * CH);
-                            const unsigned char* gsl = reinterpret_cast<const unsigned char*>(m.kv + ((size_t)(b_first + r) * NL + l) * N * (2 * D));
-                            for (int i = lane; i < rows_ * (DG::ROW_BYTES / 16); i += 32) {
-                                const int r_ = i / (DG::ROW_BYTES / 16), pc = i - r_ * (DG::ROW_BYTES / 16);
-                                const int pos = __ldg(m.mask_col + me0 + c * CH + r_);
-                                const uint4 sv = *reinterpret_cast<const uint4*>(chunk + r_ * DG::ROW_BYTES + pc * 16);
-                                const uint4 gv = ld_kv(gsl + (size_t)pos * DG::ROW_BYTES + pc * 16);
-                                if (sv.x != gv.x || sv.y != gv.y || sv.z != gv.z || sv.w != gv.w)
-                                    printf("KVMISMATCH cta %d warp %d t %d l %d r %d c %d row %d pos %d pc %d seq %u slot %u\n", blockIdx.x, warp, t, l, r, c, r_, pos, pc, sq, slot);
-                            }
-                        }
-#endif
                         attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
                         ring_release(rc, slot, lane);
                     }
@@ -723,34 +573,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 seq_base += (uint32_t)(n_own * nch);
                 cbar();
-                if constexpr (FUSED) {
-                    // ---- phase C: combine the split partials of my rows, LN2; everyone appends K|V ----
-                    for (int r = warp; r < R; r += NWC) {
-                        if (NSPLIT > 1 && r < n_own) {
-                            const float* ps = sh_split + r * NSPLIT * SPS;
-#pragma unroll
-                            for (int j = 0; j < D / 32; ++j) {
-                                const int f = lane * (D / 32) + j;
-                                float mx = -1e30f;
-#pragma unroll
-                                for (int s2 = 0; s2 < NSPLIT; ++s2) mx = fmaxf(mx, ps[s2 * SPS + f / 8]);
-                                float num = 0.f, den = 0.f;
-#pragma unroll
-                                for (int s2 = 0; s2 < NSPLIT; ++s2) {
-                                    const float wgt = exp2f(ps[s2 * SPS + f / 8] - mx);
-                                    den += wgt * ps[s2 * SPS + LPR + f / 8];
-                                    num += wgt * ps[s2 * SPS + 2 * LPR + f];
-                                }
-                                sh_h[r * HS + f] += num / den;
-                            }
-                        }
-                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
-                    }
-                    append_kv();
-                    cbar();
-                    if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
-                }
-                if (!FUSED && NSPLIT > 1) {             // combine the split partials, fixed order
+                if (NSPLIT > 1) {                       // combine the split partials, fixed order
                     for (int i = tid; i < R * D; i += NWC * 32) {
                         const int r = i / D, f = i - r * D;
                         if (r >= n_own) continue;
@@ -772,7 +595,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     cbar();
                 }
                 // ---- optional output projection (bypassed in the paper, l.107) --------------
-                if (!FUSED && m.has_wo) {
+                if (m.has_wo) {
                     {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
@@ -785,8 +608,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::NO, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
-                        (SPLIT ? seq_wc : seq_base) += DG::NO;
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
+                        seq_base += DG::NO;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
                     }
@@ -828,8 +651,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[FS2 + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
                             }
                         };
-                        gemm_ring<D / 16, NT2, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N1 / 2, (SPLIT ? seq_wc : seq_base), sh_a2, AS, warp, lane, epi);
-                        (SPLIT ? seq_wc : seq_base) += DG::N1 / 2;
+                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
+                        seq_base += DG::N1 / 2;
                     }
                     cbar();
                     // ---- FFN2 over my K-half: partial sums for all 2R rows -------------------------
@@ -843,8 +666,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
                             }
                         };
-                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N2 / 2, (SPLIT ? seq_wc : seq_base), sh_hid, FS2, warp, lane, epi);
-                        (SPLIT ? seq_wc : seq_base) += DG::N2 / 2;
+                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
+                        seq_base += DG::N2 / 2;
                     }
                     cbar();
                     {   // the peer's rows of my partial sums -> the peer's sh_xp
@@ -867,11 +690,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     cbar();
                 } else {
                     // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
-                    if constexpr (!FUSED) {
-                        for (int r = warp; r < R; r += NWC)
-                            ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
-                        cbar();
-                    }
+                    for (int r = warp; r < R; r += NWC)
+                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                    cbar();
                     // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
                     {
                         auto epi = [&](int mt, int, float (&acc)[NT][4]) {
@@ -887,11 +708,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            #ifdef FV_DBG_CHECK
-                        rcw.dbg_w = L.w1;
-#endif
-                        gemm_ring<D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N1, (SPLIT ? seq_wc : seq_base), sh_a, AS, warp, lane, epi);
-                            (SPLIT ? seq_wc : seq_base) += DG::N1;
+                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
+                            seq_base += DG::N1;
                         } else {
                             gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
                         }
@@ -909,53 +727,26 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            #ifdef FV_DBG_CHECK
-                        rcw.dbg_w = L.w2;
-#endif
-                        gemm_ring<4 * D / 16, NT, DG::TPCH, NSW, DG::CHUNK_BYTES>(rcw, DG::N2, (SPLIT ? seq_wc : seq_base), sh_hid, FS, warp, lane, epi);
-                            (SPLIT ? seq_wc : seq_base) += DG::N2;
+                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
+                            seq_base += DG::N2;
                         } else {
                             gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
                         }
                     }
                     cbar();
                     // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
-                    if constexpr (!FUSED) {
-                        for (int i = tid; i < R * D; i += NWC * 32) {
-                            const int r = i / D, f = i - r * D;
-                            float v = __ldg(L.b2 + f);
-#pragma unroll
-                            for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
-                            sh_h[r * HS + f] += v;
-                        }
-                        cbar();
-                    } else {
-                        // ---- phase R: residual of my rows, then what follows for the row: the next layer's
-                        //      LN1, or (last layer) head + draw + log q + next step's embedding + LN1 -----
-                        for (int r = warp; r < R; r += NWC) {
-#pragma unroll
-                            for (int j = 0; j < D / 32; ++j) {
-                                const int f = lane * (D / 32) + j;
-                                float v = __ldg(L.b2 + f);
-#pragma unroll
-                                for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
-                                sh_h[r * HS + f] += v;
-                            }
-                            if (l + 1 < NL) {
-                                const FvLayerDev& Ln = m.layer[l + 1];
-                                ln_row<D>(sh_h + r * HS, Ln.ln1_g, Ln.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
-                            } else {
-                                if (r < n_own) head_row(r, t, b_first, n_own);
-                                if (t + 1 < N) embed_ln1(r, t + 1);
-                            }
-                        }
-                        cbar();
+                    for (int i = tid; i < R * D; i += NWC * 32) {
+                        const int r = i / D, f = i - r * D;
+                        float v = __ldg(L.b2 + f);
+    #pragma unroll
+                        for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                        sh_h[r * HS + f] += v;
                     }
+                    cbar();
 
                 }
             }
             // ---- output head: p(+1) = softmax(z)[1] = sigmoid(z1 - z0) (Alg. 2 l.20-22) -----
-            if constexpr (!FUSED) {
             for (int r = warp; r < R; r += NWC) {
                 if (r >= n_own) continue;
                 const int b = b_first + r;
@@ -979,7 +770,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 sh_logq[tid] += (double)sh_logp[tid];
                 if (t == N - 1) a.logq[b_first + tid] = (float)sh_logq[tid];
             }
-            }
         }
         cbar();
     }
@@ -989,9 +779,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
 }  // namespace
 
 // ------------------------------------------------------------------------------ dispatch
-template <int D, int DH, int NT, bool CL, bool FUSED>
+template <int D, int DH, int NT, bool CL>
 static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
-    auto kern = fv_decode_kernel<D, DH, NT, CL, FUSED>;
+    auto kern = fv_decode_kernel<D, DH, NT, CL>;
     using DG = DecGeo<D, NT, CL>;
     const size_t smem = DG::total;
     static bool attr_set = false;                 // per instantiation
@@ -1020,21 +810,10 @@ static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n
 
 template <int D, int DH, bool CL>
 static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArgs& a, int n_sms, cudaStream_t s) {
-    const bool fused = !CL && !m.has_wo && FV_DEC_FUSED;
-    if (fused) {
-        if constexpr (!CL) {
-            switch (nt) {
-                case 1: return launch_dec<D, DH, 1, false, true>(m, a, n_sms, s);
-                case 2: return launch_dec<D, DH, 2, false, true>(m, a, n_sms, s);
-                case 4: return launch_dec<D, DH, 4, false, true>(m, a, n_sms, s);
-                default: return cudaErrorInvalidValue;
-            }
-        }
-    }
     switch (nt) {
-        case 1: return launch_dec<D, DH, 1, CL, false>(m, a, n_sms, s);
-        case 2: return launch_dec<D, DH, 2, CL, false>(m, a, n_sms, s);
-        case 4: return launch_dec<D, DH, 4, CL, false>(m, a, n_sms, s);
+        case 1: return launch_dec<D, DH, 1, CL>(m, a, n_sms, s);
+        case 2: return launch_dec<D, DH, 2, CL>(m, a, n_sms, s);
+        case 4: return launch_dec<D, DH, 4, CL>(m, a, n_sms, s);
         default: return cudaErrorInvalidValue;
     }
 }
