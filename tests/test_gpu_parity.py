@@ -223,3 +223,15 @@ def test_sample_is_reproducible_across_fresh_models():
             ref = [x.clone() for x in out]
         assert all(torch.equal(x, y) for x, y in zip(out, ref)), f"run {it} differs"
         model.close()
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 17])
+def test_tiny_sequences(N):
+    """Degenerate lengths: N = 1 (only the start token), N = 2, 3 and a ragged 17; full causal mask,
+    B = 1 and a ragged batch."""
+    w = dataclasses.replace(W.CONFIGS["cfg1"], L=N, n_sites=N)
+    for B in (1, 37):
+        model, weights, posemb, rp, col = build(w, B)
+        check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=N))
+        check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=N))
+        model.close()
