@@ -185,14 +185,14 @@ __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int row
             s[u] = ok[u] ? d : -INFINITY;
             mx = fmaxf(mx, s[u]);
         }
-        const float corr = exp2f(m - mx);
+        const float corr = fast_exp2(m - mx);
         m = mx;
         l *= corr;
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc[j] *= corr;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const float p = exp2f(s[u] - mx);
+            const float p = fast_exp2(s[u] - mx);
             l += p;
             acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
             acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
@@ -544,7 +544,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         const float m2 = __shfl_xor_sync(0xffffffffu, mm, o);
                         const float l2 = __shfl_xor_sync(0xffffffffu, ll, o);
                         const float mx = fmaxf(mm, m2);
-                        const float c1 = exp2f(mm - mx), c2 = exp2f(m2 - mx);
+                        const float c1 = fast_exp2(mm - mx), c2 = fast_exp2(m2 - mx);
                         ll = ll * c1 + l2 * c2;
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
@@ -584,7 +584,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         float num = 0.f, den = 0.f;
 #pragma unroll
                         for (int s = 0; s < NSPLIT; ++s) {
-                            const float w = exp2f(ps[s * SPS + f / 8] - mx);
+                            const float w = fast_exp2(ps[s * SPS + f / 8] - mx);
                             den += w * ps[s * SPS + LPR + f / 8];
                             num += w * ps[s * SPS + 2 * LPR + f];
                         }

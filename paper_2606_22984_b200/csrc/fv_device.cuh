@@ -44,6 +44,14 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// 2^x by the SFU alone (MUFU.EX2, denormal results flushed to zero): fast_exp2() wraps the same
+// instruction in a range check and two scalings for denormals, which a softmax weight never needs.
+__device__ __forceinline__ float fast_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -203,14 +211,14 @@ __device__ __forceinline__ void attend_range(const float* qrow, const __nv_bfloa
             s[u] = ok[u] ? d : -INFINITY;
             mx = fmaxf(mx, s[u]);
         }
-        const float corr = exp2f(m - mx);
+        const float corr = fast_exp2(m - mx);
         m = mx;
         l *= corr;
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc[j] *= corr;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const float p = exp2f(s[u] - mx);
+            const float p = fast_exp2(s[u] - mx);
             l += p;
             acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
             acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
@@ -223,7 +231,7 @@ __device__ __forceinline__ void attend_range(const float* qrow, const __nv_bfloa
         const float m2 = __shfl_xor_sync(0xffffffffu, m, o);
         const float l2 = __shfl_xor_sync(0xffffffffu, l, o);
         const float mx = fmaxf(m, m2);
-        const float c1 = exp2f(m - mx), c2 = exp2f(m2 - mx);
+        const float c1 = fast_exp2(m - mx), c2 = fast_exp2(m2 - mx);
         l = l * c1 + l2 * c2;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {

@@ -177,7 +177,7 @@ fv_forward_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ 
                         float num = 0.f, den = 0.f;
 #pragma unroll
                         for (int s = 0; s < NSPLIT; ++s) {
-                            const float w = exp2f(ps[s * SPS + f / 8] - mx);
+                            const float w = fast_exp2(ps[s * SPS + f / 8] - mx);
                             den += w * ps[s * SPS + LPR + f / 8];
                             num += w * ps[s * SPS + 2 * LPR + f];
                         }

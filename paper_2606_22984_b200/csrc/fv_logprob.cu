@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                 float corr[2];
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
-                    corr[x] = exp2f(mrow[mt][x] - mx[x]);
+                    corr[x] = fast_exp2(mrow[mt][x] - mx[x]);
                     mrow[mt][x] = mx[x];
                     lrow[mt][x] *= corr[x];
                 }
@@ -447,7 +447,7 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                 for (int n = 0; n < 2; ++n)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
-                        p[n][e] = ok[n][e] ? exp2f(sc[n][e] - mx[e >> 1]) : 0.f;
+                        p[n][e] = ok[n][e] ? fast_exp2(sc[n][e] - mx[e >> 1]) : 0.f;
                         lrow[mt][e >> 1] += p[n][e];
                     }
 #pragma unroll
