@@ -421,33 +421,40 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                     mma_bf16(sc[n], make_uint4(qa[mt][0], qa[mt][1], qa[mt][2], qa[mt][3]), kf[2 * n], kf[2 * n + 1]);
                     mma_bf16(sc[n], make_uint4(ql[mt][0], ql[mt][1], ql[mt][2], ql[mt][3]), kf[2 * n], kf[2 * n + 1]);
                 }
-                bool ok[2][4];
+                // fast path: every key of the step is allowed for all 16 queries of the tile (the inside
+                // of a sliding window) -- no per-element mask arithmetic
+                const bool full = __all_sync(0xffffffffu, (bits[mt][0] & bits[mt][1]) == 0xFFFFu);
                 float mx[2] = {mrow[mt][0], mrow[mt][1]};
+                float p[2][4];
+                float corr[2];
+                if (full) {
 #pragma unroll
-                for (int n = 0; n < 2; ++n)
+                    for (int n = 0; n < 2; ++n)
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        ok[n][e] = (bits[mt][e >> 1] >> (n * 8 + 2 * c + (e & 1))) & 1u;
-                        if (ok[n][e]) mx[e >> 1] = fmaxf(mx[e >> 1], sc[n][e]);
-                    }
+                        for (int e = 0; e < 4; ++e) mx[e >> 1] = fmaxf(mx[e >> 1], sc[n][e]);
+                } else {
+#pragma unroll
+                    for (int n = 0; n < 2; ++n)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const bool ok = (bits[mt][e >> 1] >> (n * 8 + 2 * c + (e & 1))) & 1u;
+                            sc[n][e] = ok ? sc[n][e] : -INFINITY;      // exp2(-inf - m) = 0 exactly (m is finite)
+                            mx[e >> 1] = fmaxf(mx[e >> 1], sc[n][e]);
+                        }
+                }
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
                     mx[x] = fmaxf(mx[x], __shfl_xor_sync(0xffffffffu, mx[x], 1));
                     mx[x] = fmaxf(mx[x], __shfl_xor_sync(0xffffffffu, mx[x], 2));
-                }
-                float corr[2];
-#pragma unroll
-                for (int x = 0; x < 2; ++x) {
                     corr[x] = fast_exp2(mrow[mt][x] - mx[x]);
                     mrow[mt][x] = mx[x];
                     lrow[mt][x] *= corr[x];
                 }
-                float p[2][4];
 #pragma unroll
                 for (int n = 0; n < 2; ++n)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
-                        p[n][e] = ok[n][e] ? fast_exp2(sc[n][e] - mx[e >> 1]) : 0.f;
+                        p[n][e] = fast_exp2(sc[n][e] - mx[e >> 1]);
                         lrow[mt][e >> 1] += p[n][e];
                     }
 #pragma unroll
