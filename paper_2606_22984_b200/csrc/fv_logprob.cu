@@ -314,6 +314,9 @@ __global__ void __launch_bounds__(512) lp_attn_kernel(const __grid_constant__ Lp
 //   O += P V  : P re-used from the C fragments as the A operand (bf16), V via ldmatrix.trans
 // K|V rows of the union are staged in shared memory by cp.async in chunks of 64 keys, double
 // buffered; rows are padded by 16 B so the 8 rows of an ldmatrix tile hit different banks.
+#ifndef FV_LP_PSPLIT
+#define FV_LP_PSPLIT 1      // 0: P as one bf16 (4.3 instead of 4.9 ms per layer on cfg5, but the sample/log_prob chain-rule check at 2e-4 fails)
+#endif
 constexpr int ATT_BQ = 32, ATT_UC = 64;
 
 __device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t addr) {
@@ -461,6 +464,7 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                 for (int x = 0; x < 2; ++x)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) o[mt][x][e] *= corr[e >> 1];
+#if FV_LP_PSPLIT
                 uint4 pa, pl;                              // P = hi + lo in bf16 (as q above)
                 split_bf16(p[0][0], p[0][1], pa.x, pl.x);
                 split_bf16(p[0][2], p[0][3], pa.y, pl.y);
@@ -470,6 +474,12 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                 mma_bf16(o[mt][1], pa, vf[2], vf[3]);
                 mma_bf16(o[mt][0], pl, vf[0], vf[1]);
                 mma_bf16(o[mt][1], pl, vf[2], vf[3]);
+#else
+                const uint4 pa = make_uint4(pack_bf16(p[0][0], p[0][1]), pack_bf16(p[0][2], p[0][3]),
+                                            pack_bf16(p[1][0], p[1][1]), pack_bf16(p[1][2], p[1][3]));
+                mma_bf16(o[mt][0], pa, vf[0], vf[1]);
+                mma_bf16(o[mt][1], pa, vf[2], vf[3]);
+#endif
             }
         }
         __syncthreads();                               // buffer (ch & 1) is restaged two chunks later
