@@ -16,7 +16,6 @@
 // Optional (FLASHVAN_DECODE=cluster): 2-CTA clusters in which each CTA streams only its half of
 // W_1/W_2 and applies it to the rows of both CTAs, exchanging LN2 rows and partial sums through
 // distributed shared memory (correct, measured slower: DESIGN.md 6.1).
-#include <cstdio>
 #include "fv_device.cuh"
 
 // Tuning knobs (compile time; the defaults are the measured best).
@@ -88,20 +87,10 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int who = 0, uint32_t tag = 0) {
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     const uint32_t addr = smem_u32(bar);
     uint32_t done;
-#ifdef FV_DEC_WATCHDOG
-    long long spins = 0;
-#endif
     do {
-#ifdef FV_DEC_WATCHDOG
-        if (++spins > 4000000) {
-            printf("WATCHDOG who=%d cta=%d warp=%d lane=%d tag=%u parity=%u\n", who, blockIdx.x, threadIdx.x >> 5,
-                   threadIdx.x & 31, tag, parity);
-            return;
-        }
-#endif
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
             "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
@@ -216,7 +205,7 @@ __device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32
     slot = sq % NSLOT;
     const uint32_t par = (sq / NSLOT) & 1u;
     while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
-    mbar_wait(rc.bar_full + slot, par, 2, sq);
+    mbar_wait(rc.bar_full + slot, par);
     return rc.ring + (size_t)slot * CHUNK_BYTES;
 }
 __device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
@@ -337,7 +326,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 if (lane < VW && i < n) {
                     const uint32_t sq = seq + (uint32_t)i;
                     const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                    mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
+                    mbar_wait(bar_empty + slot, par ^ 1u);
                     mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
                     bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
                              (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
@@ -406,7 +395,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             } else { r = i / nch; c = i - r * nch; }                  // sample-major
                             const uint32_t sq = seq + (uint32_t)i;
                             const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                            mbar_wait(bar_empty + slot, par ^ 1u, 1, sq);
+                            mbar_wait(bar_empty + slot, par ^ 1u);
                             const int rows = min(CH, nn - c * CH);
                             mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * DG::ROW_BYTES);
                             const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
