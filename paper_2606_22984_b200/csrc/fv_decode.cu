@@ -98,6 +98,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
             : "=r"(done) : "r"(addr), "r"(parity) : "memory");
     } while (!done);
 }
+// One bounded probe of a phase (the hardware suspends the thread for a short, implementation-defined time).
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return done != 0;
+}
 // TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier.
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
@@ -318,21 +328,31 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
+        // Chunks are armed strictly in ring order, but as soon as their slot is free: each round the lanes
+        // probe the next VW slots once and the leading run of free ones is issued.  (Waiting for all VW
+        // slots would hold back the refill of a slot until VW - 1 later chunks had been consumed as well:
+        // two or three exposed HBM round trips per attention phase instead of one.)
+        auto ready_prefix = [&](bool active, uint32_t slot, uint32_t par) {
+            const bool ok = active && mbar_test(bar_empty + slot, par ^ 1u);
+            const unsigned int bm = __ballot_sync(0xffffffffu, ok);
+            return __ffs(~bm) - 1;                           // lanes 0 .. npre-1 are all free (32 if every lane)
+        };
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
-            for (int i0 = 0; i0 < n; i0 += VW) {
+            for (int i0 = 0; i0 < n;) {
                 const int i = i0 + lane;
-                if (lane < VW && i < n) {
-                    const uint32_t sq = seq + (uint32_t)i;
-                    const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                    mbar_wait(bar_empty + slot, par ^ 1u);
+                const uint32_t sq = seq + (uint32_t)i;
+                const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                const int npre = ready_prefix(lane < VW && i < n, slot, par);
+                if (lane < npre) {
                     mbar_arrive_expect_tx(bar_full + slot, (uint32_t)DG::CHUNK_BYTES);
                     bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, src + (size_t)i * stride * DG::CHUNK_BYTES,
                              (uint32_t)DG::CHUNK_BYTES, bar_full + slot);
                 }
                 __syncwarp();
-                if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, n)));
+                i0 += npre;
+                if (lane == 0 && npre) st_release_s32(sh_issued, (int)(seq + (uint32_t)i0));
             }
             seq += (uint32_t)n;
         };
@@ -380,9 +400,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     }
                     const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
                         m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
-                    for (int i0 = 0; i0 < total; i0 += VW) {
+                    for (int i0 = 0; i0 < total;) {
                         const int i = i0 + lane;
-                        if (lane < VW && i < total) {
+                        const uint32_t sq = seq + (uint32_t)i;
+                        const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                        const int npre = ready_prefix(lane < VW && i < total, slot, par);
+                        if (lane < npre) {
                             int r, c;
                             if (FV_DEC_ORDER) {
                                 // chunk-major inside a round of GR samples (= the samples the compute
@@ -393,9 +416,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 c = rem / nk;
                                 r = k * GR + (rem - c * nk);
                             } else { r = i / nch; c = i - r * nch; }                  // sample-major
-                            const uint32_t sq = seq + (uint32_t)i;
-                            const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                            mbar_wait(bar_empty + slot, par ^ 1u);
                             const int rows = min(CH, nn - c * CH);
                             mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * DG::ROW_BYTES);
                             const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
@@ -408,7 +428,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         }
                         __syncwarp();
-                        if (lane == 0) st_release_s32(sh_issued, (int)(seq + (uint32_t)min(i0 + VW, total)));
+                        i0 += npre;
+                        if (lane == 0 && npre) st_release_s32(sh_issued, (int)(seq + (uint32_t)i0));
                     }
                     seq += (uint32_t)total;
                     if (DG::WRING) {
