@@ -335,7 +335,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         auto ready_prefix = [&](bool active, uint32_t slot, uint32_t par) {
             const bool ok = active && mbar_test(bar_empty + slot, par ^ 1u);
             const unsigned int bm = __ballot_sync(0xffffffffu, ok);
-            return __ffs(~bm) - 1;                           // lanes 0 .. npre-1 are all free (32 if every lane)
+            return bm == 0xffffffffu ? 32 : __ffs(~bm) - 1;  // lanes 0 .. npre-1 are all free
         };
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {

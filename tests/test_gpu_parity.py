@@ -159,13 +159,10 @@ def test_batch_edges_and_errors():
 
 
 # ------------------------------------------- full BASELINE sizes, bench.py's launch configuration
-@pytest.mark.parametrize("name,n_check", [("cfg2", 16), ("cfg3", 6), ("cfg4", 6), ("cfg5", 3)])
-def test_full_size_sampled_rows(name, n_check):
+def _check_sampled_rows(w, B, n_check):
     """fv_sample and fv_log_prob at the full batch and length of the BASELINE config (the launch
     geometry bench.py times: samples per CTA, ring smaller than a layer-step, several rounds per
     CTA), checked on a few samples the oracle can afford: first, last and evenly spread ones."""
-    w = W.CONFIGS[name]
-    B = w.batch
     model, weights, posemb, rp, col = build(w, B)
     u = W.make_uniforms(w, B)
     spins_g, lq_g, cp_g = model.sample(dev(u), want_cond_p=True)
@@ -190,6 +187,21 @@ def test_full_size_sampled_rows(name, n_check):
     assert torch.isfinite(lq_g).all() and torch.isfinite(lq_tf).all()
     assert (lq_g - lq_tf).abs().max().item() <= 2e-4 * max(1.0, lq_g.abs().max().item())
     model.close()
+
+
+@pytest.mark.parametrize("name,n_check", [("cfg2", 16), ("cfg3", 6), ("cfg4", 6), ("cfg5", 3)])
+def test_full_size_sampled_rows(name, n_check):
+    w = W.CONFIGS[name]
+    _check_sampled_rows(w, w.batch, n_check)
+
+
+def test_32_samples_per_cta():
+    """The largest group a CTA takes (32 samples, all 32 producer lanes armed in one round) on a short
+    d = 64 lattice, and a two-rounds-per-CTA batch."""
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=8, n_sites=64, window=8)
+    n_sms = torch.cuda.get_device_properties(0).multi_processor_count
+    _check_sampled_rows(w, 32 * n_sms, 24)
+    _check_sampled_rows(w, 32 * n_sms + 77, 24)
 
 
 def test_cluster_decode_variant(monkeypatch):
