@@ -41,7 +41,7 @@ def parse():
 
 
 # DRAM bytes of the fv_sample launch from the committed ncu capture (profiles/), keyed by (workload, batch)
-NCU_TRAFFIC = {("cfg5", 1024): 837.4e9}
+NCU_TRAFFIC = {("cfg5", 1024): 839.9e9}
 
 
 def algorithmic_kv_bytes_per_sample(w, rowptr):
@@ -280,7 +280,7 @@ def run_ours(args):
                          "algorithmic_bytes_per_launch": (rd + wr) * B,
                          "traffic": NCU_TRAFFIC.get((w.name, B)),
                          "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
-                                           "capture of this launch (profiles/r01_fv_sample_ring.md); null for "
+                                           "capture of this launch (profiles/r01_launches_cfg5.md); null for "
                                            "workloads that were not captured"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(launches), "clocks": clocks,
