@@ -242,25 +242,47 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     for (int j = warp; j < nchunks; j += NWC) {
         uint32_t slot;
         const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)j, slot)) + lane;
+        const int ks = SPLITK ? j - (j / KSP) * KSP : 0;
+        const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+        // k outer, m-tiles inner: the activation fragments of a k-step are read once and feed MPC (K = D)
+        // or two (K-part of W2: even / odd k-steps) independent accumulator chains
+        constexpr int NCH = SPLITK ? 2 : MPC;
+        float acc[NCH][NT][4];
 #pragma unroll
-        for (int mi = 0; mi < MPC; ++mi) {
-            const int mt = SPLITK ? j / KSP : j * MPC + mi;
-            const int ks = SPLITK ? j - (j / KSP) * KSP : 0;
-            float acc[NT][4];
+        for (int q = 0; q < NCH; ++q)
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) acc[nt][0] = acc[nt][1] = acc[nt][2] = acc[nt][3] = 0.f;
-            const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+            for (int nt = 0; nt < NT; ++nt) acc[q][nt][0] = acc[q][nt][1] = acc[q][nt][2] = acc[q][nt][3] = 0.f;
 #pragma unroll
-            for (int kt = 0; kt < KT; ++kt) {
-                const uint4 aw = wsm[(mi * KT + kt) * 32];
+        for (int kt = 0; kt < KT; ++kt) {
+            uint32_t b0[NT], b1[NT];
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
-                    mma_bf16(acc[nt], aw, lds32(p), lds32(p + 8));
+            for (int nt = 0; nt < NT; ++nt) {
+                const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
+                b0[nt] = lds32(p); b1[nt] = lds32(p + 8);
+            }
+            if constexpr (SPLITK) {
+                const uint4 aw = wsm[kt * 32];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) mma_bf16(acc[kt & 1][nt], aw, b0[nt], b1[nt]);
+            } else {
+#pragma unroll
+                for (int mi = 0; mi < MPC; ++mi) {
+                    const uint4 aw = wsm[(mi * KT + kt) * 32];
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) mma_bf16(acc[mi][nt], aw, b0[nt], b1[nt]);
                 }
             }
-            if (mi == MPC - 1) ring_release(rc, slot, lane);
-            epi(mt, ks, acc);
+        }
+        ring_release(rc, slot, lane);
+        if constexpr (SPLITK) {
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) acc[0][nt][e] += acc[1][nt][e];
+            epi(j / KSP, ks, acc[0]);
+        } else {
+#pragma unroll
+            for (int mi = 0; mi < MPC; ++mi) epi(j * MPC + mi, 0, acc[mi]);
         }
     }
 }
