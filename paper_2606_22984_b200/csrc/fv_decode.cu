@@ -50,8 +50,11 @@ struct DecGeo {
     static constexpr int R2 = 2 * G::R, FS2 = 2 * D + 8;
     static constexpr size_t hid2_bytes = (size_t)R2 * FS2 * 2;
     static constexpr size_t part2_bytes = (size_t)R2 * G::HS * 4;
-    static constexpr size_t big_bytes = !CL ? G::big_bytes
-                                            : (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes);
+    // the FFN2 partial sums reuse the attention-split buffer when they fit (both are dead by then)
+    static constexpr bool PART_IN_SPLIT = !CL && G::part_bytes <= G::split_bytes;
+    static constexpr size_t big_bytes = CL ? (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes)
+                                      : (!PART_IN_SPLIT ? G::big_bytes
+                                                        : (G::qkv_bytes > G::hid_bytes ? G::qkv_bytes : G::hid_bytes));
     static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
     static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
     static constexpr size_t geo_total = G::total - G::big_bytes + big_bytes + xa_bytes + xp_bytes;
@@ -59,7 +62,7 @@ struct DecGeo {
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
     static constexpr size_t fixed = (geo_total + 127) / 128 * 128;
-    static constexpr int TAB_C = 128, TAB_R = 160;        // per-step copy plan staged in smem (x2: t, t+1)
+    static constexpr int TAB_C = 48, TAB_R = 64;          // per-step copy plan staged in smem (x2: t, t+1)
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
@@ -307,8 +310,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     unsigned char* big = smem + G::h_bytes + G::a_bytes;
     float* sh_qkv = reinterpret_cast<float*>(big);
     __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
-    float* sh_part = reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
     float* sh_split = reinterpret_cast<float*>(big + DG::big_bytes);
+    float* sh_part = DG::PART_IN_SPLIT ? sh_split : reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
     double* sh_logq = reinterpret_cast<double*>(big + DG::big_bytes + G::split_bytes);
     float* sh_logp = reinterpret_cast<float*>(sh_logq + R);
     float* sh_u = sh_logp + R;
