@@ -51,13 +51,15 @@ struct DecGeo {
     static constexpr size_t hid2_bytes = (size_t)R2 * FS2 * 2;
     static constexpr size_t part2_bytes = (size_t)R2 * G::HS * 4;
     // the FFN2 partial sums reuse the attention-split buffer when they fit (both are dead by then)
-    static constexpr bool PART_IN_SPLIT = !CL && G::part_bytes <= G::split_bytes;
+    // attention-split partials exist only when several warps share a query row (R <= 8)
+    static constexpr size_t split_bytes = (NWC / G::R > 1) ? G::split_bytes : 0;
+    static constexpr bool PART_IN_SPLIT = !CL && G::part_bytes <= split_bytes;
     static constexpr size_t big_bytes = CL ? (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes)
                                       : (!PART_IN_SPLIT ? G::big_bytes
                                                         : (G::qkv_bytes > G::hid_bytes ? G::qkv_bytes : G::hid_bytes));
     static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
     static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
-    static constexpr size_t geo_total = G::total - G::big_bytes + big_bytes + xa_bytes + xp_bytes;
+    static constexpr size_t geo_total = G::total - G::big_bytes - G::split_bytes + big_bytes + split_bytes + xa_bytes + xp_bytes;
     static constexpr int CH = fv_ring_ch(D);              // KV rows per ring chunk (host plan agrees)
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
@@ -312,7 +314,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
     float* sh_split = reinterpret_cast<float*>(big + DG::big_bytes);
     float* sh_part = DG::PART_IN_SPLIT ? sh_split : reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
-    double* sh_logq = reinterpret_cast<double*>(big + DG::big_bytes + G::split_bytes);
+    double* sh_logq = reinterpret_cast<double*>(big + DG::big_bytes + DG::split_bytes);
     float* sh_logp = reinterpret_cast<float*>(sh_logq + R);
     float* sh_u = sh_logp + R;
     int* sh_tok = reinterpret_cast<int*>(sh_u + R);
