@@ -53,10 +53,15 @@ struct DecGeo {
     // the FFN2 partial sums reuse the attention-split buffer when they fit (both are dead by then)
     // attention-split partials exist only when several warps share a query row (R <= 8)
     static constexpr size_t split_bytes = (NWC / G::R > 1) ? G::split_bytes : 0;
-    static constexpr bool PART_IN_SPLIT = !CL && G::part_bytes <= split_bytes;
+    // W2 partial sums: with >= 16 rows per CTA a warp takes whole m-tiles and accumulates straight into
+    // the residual stream (gemm_ring_kparts: no buffer, 33 KB more ring at 32 rows); with 8 rows the two
+    // K-halves go to two warps (measured faster there) and their partial sums reuse the attention-split
+    // buffer, which is dead by then
+    static constexpr bool NO_PART = !CL && FV_DEC_WRING && D <= 128 && NT >= 2;
+    static constexpr bool PART_IN_SPLIT = !CL && !NO_PART && G::part_bytes <= split_bytes;
     static constexpr size_t big_bytes = CL ? (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes)
-                                      : (!PART_IN_SPLIT ? G::big_bytes
-                                                        : (G::qkv_bytes > G::hid_bytes ? G::qkv_bytes : G::hid_bytes));
+                                      : (!(NO_PART || PART_IN_SPLIT) ? G::big_bytes
+                                                                     : (G::qkv_bytes > G::hid_bytes ? G::qkv_bytes : G::hid_bytes));
     static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
     static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
     static constexpr size_t geo_total = G::total - G::big_bytes - G::split_bytes + big_bytes + split_bytes + xa_bytes + xp_bytes;
@@ -292,6 +297,46 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     }
 }
 
+// W2 GEMM (K = 4D > one chunk) with all KSP K-parts of an m-tile consumed by the SAME warp, one after the
+// other (ring order), into one accumulator: no partial-sum buffer and no separate reduction phase --
+// epi(mt, acc) applies bias and residual directly.
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, class Epi>
+__device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles, uint32_t seq0, const __nv_bfloat16* act,
+                                                 int as, int warp, int lane, Epi epi) {
+    static_assert(KT_TOTAL % TPCH == 0 && KT_TOTAL > TPCH, "K must span several chunks");
+    constexpr int KSP = KT_TOTAL / TPCH, KT = TPCH;
+    const int g = lane >> 2, c = lane & 3;
+    for (int mt = warp; mt < n_mtiles; mt += NWC) {
+        float acc[2][NT][4];                         // even / odd k-steps: two independent MMA chains
+#pragma unroll
+        for (int q = 0; q < 2; ++q)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) acc[q][nt][0] = acc[q][nt][1] = acc[q][nt][2] = acc[q][nt][3] = 0.f;
+#pragma unroll 1
+        for (int ks = 0; ks < KSP; ++ks) {
+            uint32_t slot;
+            const uint4* wsm = reinterpret_cast<const uint4*>(
+                ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)(mt * KSP + ks), slot)) + lane;
+            const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                const uint4 aw = wsm[kt * 32];
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const __nv_bfloat16* p = ab + nt * 8 * as + kt * 16;
+                    mma_bf16(acc[kt & 1][nt], aw, lds32(p), lds32(p + 8));
+                }
+            }
+            ring_release(rc, slot, lane);
+        }
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) acc[0][nt][e] += acc[1][nt][e];
+        epi(mt, acc[0]);
+    }
+}
+
 template <int D, int DH, int NT, bool CL>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ FvForwardArgs a) {
@@ -313,7 +358,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     float* sh_qkv = reinterpret_cast<float*>(big);
     __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
     float* sh_split = reinterpret_cast<float*>(big + DG::big_bytes);
-    float* sh_part = DG::PART_IN_SPLIT ? sh_split : reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
+    [[maybe_unused]] float* sh_part = DG::PART_IN_SPLIT ? sh_split     // (unused if NO_PART)
+                                                        : reinterpret_cast<float*>(big + (CL ? DG::hid2_bytes : G::hid_bytes));
     double* sh_logq = reinterpret_cast<double*>(big + DG::big_bytes + DG::split_bytes);
     float* sh_logp = reinterpret_cast<float*>(sh_logq + R);
     float* sh_u = sh_logp + R;
@@ -752,11 +798,27 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                     }
                     cbar();
-                    // ---- FFN down-projection, K split KS2 ways into partial buffers -------------
-                    {
+                    // ---- FFN down-projection + residual (Alg. 2 l.16) ---------------------------------
+                    if constexpr (DG::NO_PART) {
+                        // a warp takes whole m-tiles (both K-halves from consecutive ring chunks): the
+                        // accumulator goes straight into the residual stream
+                        auto epi = [&](int mt, float (&acc)[NT][4]) {
+                            const int f = mt * 16 + g;
+                            const float b0 = __ldg(L.b2 + f), b1 = __ldg(L.b2 + f + 8);
+#pragma unroll
+                            for (int nt = 0; nt < NT; ++nt) {
+                                float* o = sh_h + (nt * 8 + 2 * c4) * HS + f;
+                                o[0] += acc[nt][0] + b0; o[HS] += acc[nt][1] + b0;
+                                o[8] += acc[nt][2] + b1; o[HS + 8] += acc[nt][3] + b1;
+                            }
+                        };
+                        gemm_ring_kparts<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, D / 16, seq_base, sh_hid, FS, warp, lane, epi);
+                        seq_base += DG::N2;
+                        cbar();
+                    } else {
                         auto epi = [&](int mt, int ks, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
-    #pragma unroll
+#pragma unroll
                             for (int nt = 0; nt < NT; ++nt) {
                                 float* o = sh_part + ((size_t)ks * R + nt * 8 + 2 * c4) * HS + f;
                                 o[0] = acc[nt][0]; o[HS] = acc[nt][1];
@@ -769,17 +831,16 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         } else {
                             gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
                         }
+                        cbar();
+                        for (int i = tid; i < R * D; i += NWC * 32) {
+                            const int r = i / D, f = i - r * D;
+                            float v = __ldg(L.b2 + f);
+#pragma unroll
+                            for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
+                            sh_h[r * HS + f] += v;
+                        }
+                        cbar();
                     }
-                    cbar();
-                    // ---- feed-forward residual (Alg. 2 l.16) ------------------------------------
-                    for (int i = tid; i < R * D; i += NWC * 32) {
-                        const int r = i / D, f = i - r * D;
-                        float v = __ldg(L.b2 + f);
-    #pragma unroll
-                        for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
-                        sh_h[r * HS + f] += v;
-                    }
-                    cbar();
 
                 }
             }
