@@ -48,6 +48,10 @@ struct DecGeo {
     using G = Geo<D, NT>;
     // cluster mode: FFN over the 2R rows of both CTAs, hidden half (2D columns) per CTA
     static constexpr int R2 = 2 * G::R, FS2 = 2 * D + 8;
+    // q stays fp32; k|v of the step are kept as the bf16 the pool stores (append = plain copy)
+    static constexpr int QS2 = D + 4, KVS = 2 * D + 8;
+    static constexpr size_t q_bytes = (size_t)G::R * QS2 * 4;
+    static constexpr size_t qkv_bytes = q_bytes + (size_t)G::R * KVS * 2;
     static constexpr size_t hid2_bytes = (size_t)R2 * FS2 * 2;
     static constexpr size_t part2_bytes = (size_t)R2 * G::HS * 4;
     // the FFN2 partial sums reuse the attention-split buffer when they fit (both are dead by then)
@@ -59,9 +63,10 @@ struct DecGeo {
     // buffer, which is dead by then
     static constexpr bool NO_PART = !CL && FV_DEC_WRING && D <= 128 && NT >= 2;
     static constexpr bool PART_IN_SPLIT = !CL && !NO_PART && G::part_bytes <= split_bytes;
-    static constexpr size_t big_bytes = CL ? (G::qkv_bytes > hid2_bytes + part2_bytes ? G::qkv_bytes : hid2_bytes + part2_bytes)
-                                      : (!(NO_PART || PART_IN_SPLIT) ? G::big_bytes
-                                                                     : (G::qkv_bytes > G::hid_bytes ? G::qkv_bytes : G::hid_bytes));
+    static constexpr size_t big_bytes = CL ? (qkv_bytes > hid2_bytes + part2_bytes ? qkv_bytes : hid2_bytes + part2_bytes)
+                                      : (!(NO_PART || PART_IN_SPLIT)
+                                             ? (qkv_bytes > G::hid_bytes + G::part_bytes ? qkv_bytes : G::hid_bytes + G::part_bytes)
+                                             : (qkv_bytes > G::hid_bytes ? qkv_bytes : G::hid_bytes));
     static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
     static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
     static constexpr size_t geo_total = G::total - G::big_bytes - G::split_bytes + big_bytes + split_bytes + xa_bytes + xp_bytes;
@@ -69,7 +74,7 @@ struct DecGeo {
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
     static constexpr size_t fixed = (geo_total + 127) / 128 * 128;
-    static constexpr int TAB_C = 48, TAB_R = 64;          // per-step copy plan staged in smem (x2: t, t+1)
+    static constexpr int TAB_C = 48, TAB_R = 48;          // per-step copy plan staged in smem (x2: t, t+1)
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
@@ -159,7 +164,6 @@ __device__ __forceinline__ int ld_acquire_s32(const int* p) {
 __device__ __forceinline__ void st_release_s32(int* p, int v) {
     asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
-__device__ __forceinline__ float bf16_round(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
 
 // Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
 // PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
@@ -343,7 +347,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     using G = Geo<D, NT>;
     using DG = DecGeo<D, NT, CL>;
     [[maybe_unused]] constexpr int R2 = DG::R2, FS2 = DG::FS2, NT2 = 2 * NT;
-    constexpr int R = G::R, HS = G::HS, AS = G::AS, QS = G::QS, FS = G::FS, KS2 = G::KS2;
+    constexpr int R = G::R, HS = G::HS, AS = G::AS, FS = G::FS, KS2 = G::KS2;
     constexpr int NSPLIT = (NWC / R) > 1 ? (NWC / R) : 1;    // warps cooperating on one query row
     constexpr int LPR = D / 8, LPH = DH / 8;
     constexpr int SPS = D + 2 * LPR;                          // floats per split-partial slot
@@ -355,7 +359,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     float* sh_h = reinterpret_cast<float*>(smem);
     __nv_bfloat16* sh_a = reinterpret_cast<__nv_bfloat16*>(smem + G::h_bytes);
     unsigned char* big = smem + G::h_bytes + G::a_bytes;
-    float* sh_qkv = reinterpret_cast<float*>(big);
+    float* sh_q = reinterpret_cast<float*>(big);
+    __nv_bfloat16* sh_kv = reinterpret_cast<__nv_bfloat16*>(big + DG::q_bytes);
+    constexpr int QS2 = DG::QS2, KVS = DG::KVS;
     __nv_bfloat16* sh_hid = reinterpret_cast<__nv_bfloat16*>(big);
     float* sh_split = reinterpret_cast<float*>(big + DG::big_bytes);
     [[maybe_unused]] float* sh_part = DG::PART_IN_SPLIT ? sh_split     // (unused if NO_PART)
@@ -561,9 +567,16 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         const float b0 = __ldg(L.bqkv + f), b1 = __ldg(L.bqkv + f + 8);
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt) {
-                            float* o = sh_qkv + (nt * 8 + 2 * c4) * QS + f;
-                            o[0] = acc[nt][0] + b0; o[QS] = acc[nt][1] + b0;
-                            o[8] = acc[nt][2] + b1; o[QS + 8] = acc[nt][3] + b1;
+                            const int row = nt * 8 + 2 * c4;
+                            if (f < D) {                         // whole m-tile is q (warp-uniform)
+                                float* o = sh_q + row * QS2 + f;
+                                o[0] = acc[nt][0] + b0; o[QS2] = acc[nt][1] + b0;
+                                o[8] = acc[nt][2] + b1; o[QS2 + 8] = acc[nt][3] + b1;
+                            } else {
+                                __nv_bfloat16* o = sh_kv + row * KVS + (f - D);
+                                o[0] = __float2bfloat16_rn(acc[nt][0] + b0); o[KVS] = __float2bfloat16_rn(acc[nt][1] + b0);
+                                o[8] = __float2bfloat16_rn(acc[nt][2] + b1); o[KVS + 8] = __float2bfloat16_rn(acc[nt][3] + b1);
+                            }
                         }
                     };
                     if constexpr (DG::WRING) {
@@ -578,10 +591,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
                     const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
                     if (r >= n_own) continue;
-                    const float* s = sh_qkv + r * QS + D + ch * 8;
-                    uint4 v;
-                    v.x = pack_bf16(s[0], s[1]); v.y = pack_bf16(s[2], s[3]);
-                    v.z = pack_bf16(s[4], s[5]); v.w = pack_bf16(s[6], s[7]);
+                    const uint4 v = *reinterpret_cast<const uint4*>(sh_kv + r * KVS + ch * 8);
                     __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
                     *reinterpret_cast<uint4*>(dst) = v;
                 }
@@ -594,7 +604,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
                     if (r >= n_own) continue;
                     const float qs = kLog2e * rsqrtf((float)DH);
-                    const float* qrow = sh_qkv + r * QS;
+                    const float* qrow = sh_q + r * QS2;
+                    const __nv_bfloat16* kvrow = sh_kv + r * KVS;
                     float q[8], acc[8];
 #pragma unroll
                     for (int j = 0; j < 8; ++j) q[j] = qrow[sub * 8 + j] * qs;
@@ -604,13 +615,13 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     if (sp == 0) {                       // row t itself, as the pool stores it (bf16)
                         float d = 0.f;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) d += q[j] * bf16_round(qrow[D + sub * 8 + j]);
+                        for (int j = 0; j < 8; ++j) d += q[j] * __bfloat162float(kvrow[sub * 8 + j]);
 #pragma unroll
                         for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
                         if (rg == 0) {
                             mm = d; ll = 1.f;
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) acc[j] = bf16_round(qrow[2 * D + sub * 8 + j]);
+                            for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + sub * 8 + j]);
                         }
                     }
                     for (int c = sp; c < nch; c += NSPLIT) {
