@@ -595,10 +595,10 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
                     *reinterpret_cast<uint4*>(dst) = v;
                 }
-                // the producer reads these rows through the async proxy (cp.async.bulk)
+                // the producer reads these rows through the async proxy (cp.async.bulk); they are first needed
+                // one step later, so the append shares its barrier with the attention phase and is published
+                // after it
                 asm volatile("fence.proxy.async.global;\n" ::: "memory");
-                cbar();
-                if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
                 for (int task = warp; task < R * NSPLIT; task += NWC) {
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
@@ -667,6 +667,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 seq_base += (uint32_t)(n_own * nch);
                 cbar();
+                if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 if (NSPLIT > 1) {                       // combine the split partials, fixed order
                     for (int i = tid; i < R * D; i += NWC * 32) {
                         const int r = i / D, f = i - r * D;
