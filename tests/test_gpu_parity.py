@@ -247,3 +247,21 @@ def test_tiny_sequences(N):
         check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=N))
         check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=N))
         model.close()
+
+
+@pytest.mark.parametrize("density,d_model,n_heads", [(0.5, 128, 8), (0.15, 64, 4)])
+def test_random_csr_masks(density, d_model, n_heads):
+    """Arbitrary (non-lattice) CSR masks: every row a random subset of the earlier positions plus
+    itself -- many isolated entries, i.e. more runs per step than the kernel's shared-memory copy
+    plan holds (falls back to the plan in global memory), and unions that span the whole prefix in
+    the block attention of fv_log_prob."""
+    N, B = 160, 21
+    w = dataclasses.replace(W.CONFIGS["cfg3"], L=N, n_sites=N, d_model=d_model, n_heads=n_heads, n_layers=2)
+    rng = np.random.default_rng(7)
+    rows = [np.concatenate([np.nonzero(rng.random(t) < density)[0], [t]]).astype(np.int32) for t in range(N)]
+    rp = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int32)
+    col = np.concatenate(rows).astype(np.int32)
+    model, weights, posemb, rp, col = build(w, B, mask=(rp, col))
+    check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=5))
+    check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=5))
+    model.close()
