@@ -31,6 +31,9 @@
 #ifndef FV_DEC_WRING
 #define FV_DEC_WRING 1      // 1: GEMM weights stream through the shared-memory ring (TMA), 0: LDG from L2
 #endif
+#ifndef FV_DEC_KVLSU
+#define FV_DEC_KVLSU 0      // 1: the KV rows are copied by a second producer warp with cp.async (LSU), the weights by TMA
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -39,7 +42,7 @@ namespace {
 using namespace fvdev;
 
 constexpr int NWC = 16;                       // compute warps
-constexpr int NTHREADS = NWC * 32 + 32;       // + 1 producer warp
+constexpr int NTHREADS = NWC * 32 + (FV_DEC_KVLSU ? 64 : 32);   // + producer warp(s)
 constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
 
 // CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
@@ -376,7 +379,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + DG::fixed);
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
-    int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
+    int* sh_issued = sh_app + 1;                                   // ring chunks armed so far (weights if KVLSU)
+    int* sh_issued_k = FV_DEC_KVLSU ? sh_app + 6 : sh_issued;      // KV chunks armed so far (own producer)
     uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 2);     // [2] cluster exchange barriers (LN2 rows, partials)
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
     int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
@@ -389,6 +393,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
         *sh_app = 0;
         *sh_issued = 0;
+        *sh_issued_k = 0;
         if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
@@ -403,7 +408,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // Lanes work on VW consecutive chunks of the ring at once (one chunk per lane: wait for the
     // slot, arm the mbarrier, one bulk copy per run).  VW <= NSLOT, so a lane only ever waits
     // on a chunk issued in an earlier round -- no circular wait with the consumers.
-    if (warp == NWC) {
+    if (warp >= NWC) {
+        // KVLSU: warp NWC streams the weights by TMA, warp NWC + 1 copies the KV rows with cp.async (a second
+        // copy engine).  Both walk the same chunk sequence; each arms a group only after the other has armed
+        // everything before it, so a slot is never armed more than one round ahead of its barrier.
+        const bool is_tma = warp == NWC, is_lsu = FV_DEC_KVLSU && warp == NWC + 1;
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
@@ -418,6 +427,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         };
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
+            if (!is_tma) {                                   // the KV producer only keeps count
+                seq += (uint32_t)n;
+                if (lane == 0) st_release_s32(sh_issued_k, (int)seq);
+                return;
+            }
+            if (FV_DEC_KVLSU) while ((int)((uint32_t)ld_acquire_s32(sh_issued_k) - seq) < 0) __nanosleep(20);
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
             for (int i0 = 0; i0 < n;) {
                 const int i = i0 + lane;
@@ -462,9 +477,15 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 return p;
             };
-            Plan cur = stage_plan(0);
+            const bool kv_mine = FV_DEC_KVLSU ? is_lsu : true;       // this warp copies the KV rows
+            auto count_plan = [&](int t) {                           // chunk count only (the other producer)
+                Plan p{0, 0, 0, nullptr, nullptr};
+                if (t < N) p.nch = __ldg(m.chunk_ptr + t + 1) - __ldg(m.chunk_ptr + t);
+                return p;
+            };
+            Plan cur = kv_mine ? stage_plan(0) : count_plan(0);
             for (int t = 0; t < N; ++t) {
-                const Plan nxt = stage_plan(t + 1);
+                const Plan nxt = kv_mine ? stage_plan(t + 1) : count_plan(t + 1);
                 const int nch = cur.nch, nn = cur.nn;
                 const int32_t* cptr = cur.cptr;
                 const int2* rptr = cur.rptr;
@@ -472,13 +493,53 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
                     if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
-                    if (total > 0) {
+                    if (total > 0 && kv_mine) {
                         // rows < t of layer l are complete once step t-1 has appended at layer l
                         const int need = (it * N + (t - 1)) * NL + l + 1;
                         while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
                     }
                     const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
                         m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
+                    if (FV_DEC_KVLSU && is_tma) {
+                        // not mine: all weight chunks before seq + total are armed
+                        if (lane == 0 && total) st_release_s32(sh_issued, (int)(seq + (uint32_t)total));
+                    } else if (is_lsu) {
+                        // ---- cp.async (LSU) copies, one chunk after the other, the whole warp per chunk ----
+                        constexpr int PR = DG::ROW_BYTES / 16;                // 16-byte pieces per row
+                        if (total) while ((int)((uint32_t)ld_acquire_s32(sh_issued) - seq) < 0) __nanosleep(20);
+                        for (int i = 0; i < total; ++i) {
+                            int r, c;
+                            if (FV_DEC_ORDER) {
+                                const int k = i / (GR * nch), rem = i - k * GR * nch;
+                                const int nk = min(GR, n_own - k * GR);
+                                c = rem / nk;
+                                r = k * GR + (rem - c * nk);
+                            } else { r = i / nch; c = i - r * nch; }
+                            const uint32_t sq = seq + (uint32_t)i;
+                            const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                            if (lane == 0) mbar_wait(bar_empty + slot, par ^ 1u);
+                            __syncwarp();
+                            const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
+                            const uint32_t dst = smem_u32(ring + (size_t)slot * DG::CHUNK_BYTES);
+                            const int j1 = cptr[c + 1];
+                            for (int j = cptr[c]; j < j1; ++j) {
+                                const int2 run = rptr[j];
+                                const int npc = (run.y & 0xffff) * PR;
+                                const unsigned char* rs = src + (size_t)run.x * DG::ROW_BYTES;
+                                const uint32_t rd = dst + (uint32_t)(run.y >> 16) * DG::ROW_BYTES;
+                                for (int pc = lane; pc < npc; pc += 32)
+                                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(rd + pc * 16), "l"(rs + (size_t)pc * 16) : "memory");
+                            }
+                            // the chunk's full barrier: +1 pending per lane until that lane's copies have landed,
+                            // then the one counted arrival
+                            asm volatile("cp.async.mbarrier.arrive.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar_full + slot)) : "memory");
+                            __syncwarp();
+                            if (lane == 0) {
+                                mbar_arrive(bar_full + slot);
+                                st_release_s32(sh_issued_k, (int)(sq + 1));
+                            }
+                        }
+                    } else
                     for (int i0 = 0; i0 < total;) {
                         const int i = i0 + lane;
                         const uint32_t sq = seq + (uint32_t)i;
@@ -534,7 +595,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     const int rg = lane / LPR, sub = lane % LPR;
     uint32_t seq_base = 0;
     int it = 0;
-    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
+    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};          // weight chunks
+    const RingCtx rck{ring, bar_full, bar_empty, sh_issued_k};       // KV chunks (armed by their own producer if KVLSU)
     for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
         const int unit = CL ? wu * 2 + (int)crank : wu;
         const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
@@ -629,7 +691,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         const uint32_t sq = seq_base + (uint32_t)(FV_DEC_ORDER ? kr * GR * nch + c * nk + (r - kr * GR)
                                                                                : r * nch + c);
                         uint32_t slot;
-                        const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
+                        const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rck, sq, slot);
                         attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
                         ring_release(rc, slot, lane);
                     }
