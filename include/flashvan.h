@@ -111,6 +111,24 @@ int fv_free_energy(int32_t B, const float* E, const float* logq, double temperat
 
 void fv_destroy_model(fv_model* m);
 
+/* Build the paper's attention mask from the coupling graph: the ordered Markov boundary of every vertex
+ * (Sec. IV.A.1, Eq. 12-13), i.e. the past vertices j < i adjacent to i or joined to i
+ * by a path through future vertices (> i) only; a sliding window of width W >= d_max contains it
+ * (Eq. S1).  Host-only call, no device work.
+ *   n: number of vertices, numbered in sampling order.  edge_a, edge_b [host] n_edges undirected edges
+ *       (duplicates allowed; a self loop or an index outside [0, n) is FV_ERR_BAD_ARG).
+ *   position_space = 0: row i = boundary(i) in vertex indices, ascending (may be empty).
+ *   position_space = 1: row t = {j + 1 : j in boundary(t)} U {t}, ascending -- the mask_rowptr / mask_col
+ *       fv_create_model takes (position j + 1 carries spin j; reading A11).
+ *   out_rowptr [host] n + 1 (always written).  out_col [host] room for `cap` entries; if cap is smaller
+ *       than the number of entries needed, nothing is written to out_col and FV_ERR_BAD_ARG is returned
+ *       with *nnz set, so a first call with cap = 0 sizes the second.  More than 2^31 - 1 entries is
+ *       FV_ERR_BAD_SHAPE.
+ *   nnz [host, may be NULL]: entries needed.  d_max [host, may be NULL]: max_i max_{j in boundary(i)} (i - j). */
+int fv_markov_mask(int32_t n, int64_t n_edges, const int32_t* edge_a, const int32_t* edge_b,
+                   int32_t position_space, int32_t* out_rowptr, int32_t* out_col, int64_t cap,
+                   int64_t* nnz, int32_t* d_max);
+
 /* Expected n_weights for a configuration (the layout above); < 0 on a bad shape. */
 int64_t fv_n_weights(const fv_config* cfg);
 

@@ -17,7 +17,7 @@ _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.s
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
-           "fv_last_error"]
+           "fv_last_error", "fv_markov_mask"]
 
 
 class FvConfig(ctypes.Structure):
@@ -56,6 +56,7 @@ def lib() -> ctypes.CDLL:
         L.fv_kv_bytes.restype = i64
         L.fv_launch_count.restype = i64
         L.fv_last_error.restype = ctypes.c_char_p
+        L.fv_markov_mask.argtypes = [i32, i64, vp, vp, i32, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(i32)]
         _lib = L
     return _lib
 
@@ -180,3 +181,24 @@ def free_energy(E, logq, temperature: float, out=None):
     _check(lib().fv_free_energy(E.numel(), E.data_ptr(), logq.data_ptr(), float(temperature),
                                 res.data_ptr(), _stream()), "fv_free_energy")
     return res
+
+
+def markov_mask(n: int, edge_a, edge_b, position_space: bool = True):
+    """Ordered Markov boundary of every vertex as CSR (host numpy in, host numpy out): the mask
+    create_model takes when position_space, else the boundary sets themselves.  Returns
+    (rowptr int32 [n+1], col int32 [nnz], d_max)."""
+    import numpy as np
+    a = np.ascontiguousarray(edge_a, dtype=np.int32)
+    b = np.ascontiguousarray(edge_b, dtype=np.int32)
+    if a.shape != b.shape or a.ndim != 1:
+        raise FlashVanError("markov_mask: edge_a and edge_b must be 1-D arrays of one length")
+    rowptr = np.zeros(n + 1, dtype=np.int32)
+    nnz, dmax = ctypes.c_int64(0), ctypes.c_int32(0)
+    args = (n, a.size, a.ctypes.data if a.size else None, b.ctypes.data if b.size else None, int(bool(position_space)))
+    rc = lib().fv_markov_mask(*args, rowptr.ctypes.data, None, 0, ctypes.byref(nnz), ctypes.byref(dmax))
+    if rc != 0 and nnz.value == 0:
+        _check(rc, "fv_markov_mask")
+    col = np.zeros(max(nnz.value, 1), dtype=np.int32)
+    _check(lib().fv_markov_mask(*args, rowptr.ctypes.data, col.ctypes.data, nnz.value, ctypes.byref(nnz),
+                                ctypes.byref(dmax)), "fv_markov_mask")
+    return rowptr, col[:nnz.value], dmax.value

@@ -309,6 +309,44 @@ void fv_destroy_model(fv_model* m) {
     delete m;
 }
 
+// Ordered Markov boundary -> mask rows (fv_mask.cu does the graph work).
+int fv_markov_mask(int32_t n, int64_t n_edges, const int32_t* edge_a, const int32_t* edge_b,
+                   int32_t position_space, int32_t* out_rowptr, int32_t* out_col, int64_t cap,
+                   int64_t* nnz, int32_t* d_max) {
+    if (n <= 0 || n_edges < 0 || (n_edges > 0 && (!edge_a || !edge_b)) || !out_rowptr || cap < 0 ||
+        (cap > 0 && !out_col) || (position_space != 0 && position_space != 1))
+        return fail(FV_ERR_BAD_ARG, "fv_markov_mask: bad argument");
+    std::vector<std::vector<int32_t>> rows;
+    std::string err;
+    if (fv_markov_rows(n, n_edges, edge_a, edge_b, rows, err) != 0) return fail(FV_ERR_BAD_ARG, "fv_markov_mask: " + err);
+    int64_t total = 0;
+    int32_t dm = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        const std::vector<int32_t>& r = rows[i];
+        if (!r.empty()) dm = std::max(dm, i - r.front());
+        // position space: j + 1 for every boundary vertex, and t itself exactly once
+        total += position_space ? (int64_t)r.size() + ((!r.empty() && r.back() == i - 1) ? 0 : 1) : (int64_t)r.size();
+    }
+    if (nnz) *nnz = total;
+    if (d_max) *d_max = dm;
+    if (total > 0x7fffffffLL) return fail(FV_ERR_BAD_SHAPE, "fv_markov_mask: more than 2^31 - 1 mask entries");
+    int64_t at = 0;
+    out_rowptr[0] = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        const std::vector<int32_t>& r = rows[i];
+        const int64_t len = position_space ? (int64_t)r.size() + ((!r.empty() && r.back() == i - 1) ? 0 : 1) : (int64_t)r.size();
+        if (total <= cap) {
+            for (int32_t j : r)
+                if (!position_space) out_col[at++] = j;
+                else if (j + 1 < i) out_col[at++] = j + 1;
+            if (position_space) out_col[at++] = i;
+        }
+        out_rowptr[i + 1] = (int32_t)(out_rowptr[i] + len);
+    }
+    if (total > cap) return fail(FV_ERR_BAD_ARG, "fv_markov_mask: out_col holds " + std::to_string(cap) + " entries, " + std::to_string(total) + " needed");
+    return FV_OK;
+}
+
 // Launch geometry of the persistent forward kernel.
 // SAMPLE: one CTA per SM; B samples are cut into groups of S <= 32 so that the number of groups
 // is (a multiple of) the SM count; NT = ceil(S/8) rounded to {1,2,4} n8-tiles per mma.

@@ -4,6 +4,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <string>
+#include <vector>
+
 #define FV_MAX_LAYERS 16
 
 // Hidden columns per chunk of the fused FFN of fv_logprob.cu (host image packer and kernel must agree).
@@ -89,3 +92,8 @@ cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const floa
                                    cudaStream_t s);
 cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out,
                                   cudaStream_t s);
+
+// fv_mask.cu: rows[i] = ordered Markov boundary of vertex i, ascending; -1 and a
+// message in err on a bad edge.
+int fv_markov_rows(int32_t n, int64_t n_edges, const int32_t* edge_a, const int32_t* edge_b,
+                   std::vector<std::vector<int32_t>>& rows, std::string& err);

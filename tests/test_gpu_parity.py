@@ -265,3 +265,24 @@ def test_random_csr_masks(density, d_model, n_heads):
     check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=5))
     check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=5))
     model.close()
+
+
+@pytest.mark.parametrize("periodic", [False, True])
+def test_markov_boundary_mask_from_the_library(periodic):
+    """The paper's own mask: ordered Markov boundary of a 12 x 12 lattice built by
+    fv_markov_mask, fed to fv_create_model; sample and log_prob against the fp64 reference under the
+    same mask.  Periodic rows hold two runs (the first lattice row and the sliding cut)."""
+    L, B = 12, 19
+    N = L * L
+    edges = [(r * L + c, r * L + c + 1) for r in range(L) for c in range(L - 1)]
+    edges += [(r * L + c, (r + 1) * L + c) for r in range(L - 1) for c in range(L)]
+    if periodic:
+        edges += [(r * L, r * L + L - 1) for r in range(L)] + [(c, (L - 1) * L + c) for c in range(L)]
+    e = np.asarray(edges, dtype=np.int32)
+    rp, col, dmax = fv.markov_mask(N, e[:, 0], e[:, 1], position_space=True)
+    assert dmax == (N - L if periodic else L)
+    w = dataclasses.replace(W.CONFIGS["cfg5"], L=L, n_sites=N, n_layers=2)
+    model, weights, posemb, rp, col = build(w, B, mask=(rp, col))
+    check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=3))
+    check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=3))
+    model.close()

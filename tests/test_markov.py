@@ -113,3 +113,103 @@ def test_oracle_open_3d_window():
 def test_oracle_mask_rows():
     rowptr, col = OM.boundary_to_mask_csr([[], [0], [], [0, 1]])
     assert rowptr.tolist() == [0, 1, 2, 3, 6] and col.tolist() == [0, 1, 2, 1, 2, 3]
+
+
+# ------------------------------------------------------------------ the library's builder against the oracle
+
+def _lib_rows(n, edges, position_space):
+    from paper_2606_22984_b200 import binding as fv
+    from paper_2606_22984_b200 import build as fvbuild
+    fvbuild.build()
+    e = np.asarray(list(edges), dtype=np.int32).reshape(-1, 2)
+    return fv.markov_mask(n, e[:, 0], e[:, 1], position_space)
+
+
+def _oracle_csr(boundary):
+    rowptr = np.cumsum([0] + [len(b) for b in boundary]).astype(np.int32)
+    col = np.asarray([j for b in boundary for j in b], dtype=np.int32)
+    return rowptr, col
+
+
+CASES = [("open2d_L8", 64, OM.lattice_edges(8, 2, False)),
+         ("periodic2d_L8", 64, OM.lattice_edges(8, 2, True)),
+         ("periodic2d_L16", 256, OM.lattice_edges(16, 2, True)),
+         ("open3d_L4", 64, OM.lattice_edges(4, 3, False)),
+         ("periodic3d_L4", 64, OM.lattice_edges(4, 3, True)),
+         ("chain", 17, [(i, i + 1) for i in range(16)]),
+         ("complete", 33, list(itertools.combinations(range(33), 2))),
+         ("no_edges", 5, []),
+         ("single_vertex", 1, [])]
+
+
+@pytest.mark.parametrize("name,n,edges", CASES, ids=[c[0] for c in CASES])
+def test_library_matches_oracle(name, n, edges):
+    boundary = OM.ordered_markov_boundary(n, edges)
+    rowptr, col, dmax = _lib_rows(n, edges, position_space=False)
+    want_ptr, want_col = _oracle_csr(boundary)
+    assert np.array_equal(rowptr, want_ptr) and np.array_equal(col, want_col)
+    assert dmax == OM.d_max(boundary)
+    rowptr, col, _ = _lib_rows(n, edges, position_space=True)
+    want_ptr, want_col = OM.boundary_to_mask_csr(boundary)
+    assert np.array_equal(rowptr, want_ptr) and np.array_equal(col, want_col)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_library_matches_oracle_on_random_graphs_and_orderings(seed):
+    """Random sparse graphs, a random relabelling of a lattice (a non-raster ordering), duplicate and
+    reversed edges."""
+    rng = np.random.default_rng(500 + seed)
+    n = int(rng.integers(2, 120))
+    edges = _random_graph(rng, n, float(rng.choice([0.02, 0.05, 0.2])))
+    edges += [(b, a) for a, b in edges[::3]]                         # reversed duplicates
+    if seed % 2:
+        perm = rng.permutation(64)
+        edges = [(int(perm[a]), int(perm[b])) for a, b in OM.lattice_edges(8, 2, True)]
+        n = 64
+    boundary = OM.ordered_markov_boundary(n, edges)
+    rowptr, col, dmax = _lib_rows(n, edges, position_space=False)
+    want_ptr, want_col = _oracle_csr(boundary)
+    assert np.array_equal(rowptr, want_ptr) and np.array_equal(col, want_col) and dmax == OM.d_max(boundary)
+
+
+def test_library_mask_is_accepted_shape_for_cfg5_lattice():
+    """Full size: 2D periodic L = 64 (the cfg5 lattice).  Properties that hold at any size: rows ascending and
+    unique, last entry == t, every direct past neighbour present, |row| <= 2L + 1, window 2L... contains it."""
+    L = 64
+    edges = OM.lattice_edges(L, 2, True)
+    rowptr, col, dmax = _lib_rows(L * L, edges, position_space=True)
+    assert rowptr[0] == 0 and rowptr[-1] == len(col)
+    assert int(np.diff(rowptr).max()) <= 2 * L + 1
+    assert dmax == L * L - L                                     # the first row stays visible up to the last row
+    nbr = [[] for _ in range(L * L)]
+    for a, b in edges:
+        nbr[b].append(a)
+    for t in range(L * L):
+        row = col[rowptr[t]:rowptr[t + 1]]
+        assert row[-1] == t and np.all(np.diff(row) > 0) and row[0] >= 0
+        assert all((j + 1 in row) for j in nbr[t] if j < t)
+    # sampled rows against the oracle's definition (one graph search each)
+    sample = [0, 1, L - 1, L, L + 1, 2 * L + 5, 2000, L * L - L - 1, L * L - L, L * L - 2, L * L - 1]
+    nb = [set() for _ in range(L * L)]
+    for a, b in edges:
+        nb[a].add(b)
+        nb[b].add(a)
+    for t in sample:
+        found, seen, stack = set(), {t}, [t]
+        while stack:
+            v = stack.pop()
+            for u in nb[v]:
+                if u < t:
+                    found.add(u)
+                elif u not in seen:
+                    seen.add(u)
+                    stack.append(u)
+        assert col[rowptr[t]:rowptr[t + 1]].tolist() == sorted({j + 1 for j in found} | {t})
+
+
+def test_library_rejects_bad_edges():
+    from paper_2606_22984_b200 import binding as fv
+    with pytest.raises(fv.FlashVanError):
+        _lib_rows(4, [(0, 4)], False)
+    with pytest.raises(fv.FlashVanError):
+        _lib_rows(4, [(2, 2)], False)
