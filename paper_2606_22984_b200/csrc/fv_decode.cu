@@ -34,6 +34,9 @@
 #ifndef FV_DEC_KVLSU
 #define FV_DEC_KVLSU 0      // 1: the KV rows are copied by a second producer warp with cp.async (LSU), the weights by TMA
 #endif
+#ifndef FV_DEC_KV_EVICT_FIRST
+#define FV_DEC_KV_EVICT_FIRST 1   // KV rows are read with the L2 evict_first policy
+#endif
 #ifndef FV_DEC_SLOTS
 #define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
 #endif
@@ -130,6 +133,11 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// The same with an L2 eviction policy (createpolicy) attached to the read.
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
 }
 // ---- 2-CTA cluster plumbing (distributed shared memory) -------------------------------------
 __device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
@@ -413,6 +421,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         // copy engine).  Both walk the same chunk sequence; each arms a group only after the other has armed
         // everything before it, so a slot is never armed more than one round ahead of its barrier.
         const bool is_tma = warp == NWC, is_lsu = FV_DEC_KVLSU && warp == NWC + 1;
+        // The KV rows stream through L2 once per step (one step of the whole batch touches more bytes than L2
+        // holds, so none of them survives until its next use): read them evict_first so that they do not push out
+        // the GEMM weights every CTA re-reads.  cfg5: 265.6 -> 258.6 ms; a kept (evict_last) fraction of the rows
+        // or evict_last on the weights adds nothing.
+        uint64_t kv_pol = 0;
+        if (FV_DEC_KV_EVICT_FIRST) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(kv_pol));
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
@@ -563,8 +577,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             const int j1 = cptr[c + 1];
                             for (int j = cptr[c]; j < j1; ++j) {
                                 const int2 run = rptr[j];
-                                bulk_g2s(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
-                                         (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot);
+                                if (FV_DEC_KV_EVICT_FIRST)
+                                    bulk_g2s_hint(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
+                                                  (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot, kv_pol);
+                                else
+                                    bulk_g2s(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
+                                             (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot);
                             }
                         }
                         __syncwarp();
