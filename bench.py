@@ -41,7 +41,7 @@ def parse():
 
 
 # DRAM bytes of the fv_sample launch from the committed ncu capture (profiles/), keyed by (workload, batch)
-NCU_TRAFFIC = {("cfg5", 1024): 839.9e9}
+NCU_TRAFFIC = {("cfg5", 1024): 642.0e9}
 
 
 def algorithmic_kv_bytes_per_sample(w, rowptr):
