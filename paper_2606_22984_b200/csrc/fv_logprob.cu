@@ -600,6 +600,14 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
             unsigned char* w2 = sW + (int)(gch & 1) * G::WBUF + G::W1_BYTES;
             // GEMM 1 of this chunk done; tcgen05 ops of one thread complete in issue order, so the
             // previous chunk's GEMM 2 is done too: H and the other weight buffer are free
+            // this warp's 32 bias values of the chunk are fetched before the wait, not after it
+            static_assert(G::HC / 32 == NCG_F, "one 32-column block per warp and chunk");
+            float4 bpre[8];
+            {
+                const float4* b1 = reinterpret_cast<const float4*>(a.bias + j * G::HC + (warp >> 2) * 32);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) bpre[c] = __ldg(b1 + c);
+            }
             umma::mbar_wait(&bar_m1, ph1);
             ph1 ^= 1;
             umma::fence_after_sync();
@@ -611,10 +619,9 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
                 for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG_F) {
                     float v[32];
                     umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
-                    const float4* b1 = reinterpret_cast<const float4*>(a.bias + j * G::HC + cb * 32);
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        const float4 ba = __ldg(b1 + 2 * c), bb = __ldg(b1 + 2 * c + 1);
+                        const float4 ba = bpre[2 * c], bb = bpre[2 * c + 1];
                         uint32_t p[4];
                         p[0] = pack_bf16(gelu_fast(v[c * 8 + 0] + ba.x), gelu_fast(v[c * 8 + 1] + ba.y));
                         p[1] = pack_bf16(gelu_fast(v[c * 8 + 2] + ba.z), gelu_fast(v[c * 8 + 3] + ba.w));
