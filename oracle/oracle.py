@@ -134,6 +134,21 @@ def free_energy(E, logq, beta):
     return float(f.mean()), float(f.std())
 
 
+def overlap(spins_a, spins_b):
+    """Replica overlap (Eq. 9): dot_b = sum_i a_bi * c_bi, an explicit loop over sites in exact
+    integers; q_b = dot_b / N.  Returns (dot int64 [B], hist int64 [N + 1]) with hist[(dot + N) / 2] counting
+    the samples at each of the N + 1 values -N, -N + 2, ..., N the sum can take (p(q) = hist / B)."""
+    a, c = _c(spins_a, np.int8), _c(spins_b, np.int8)
+    B, N = a.shape
+    dot = np.zeros(B, np.int64)
+    for i in range(N):
+        dot += a[:, i].astype(np.int64) * c[:, i].astype(np.int64)
+    hist = np.zeros(N + 1, np.int64)
+    for b in range(B):
+        hist[(int(dot[b]) + N) // 2] += 1
+    return dot, hist
+
+
 def param_count(vocab, n_seq, d_token, d_model, n_layers, ffn_mult=4, has_wo=0):
     """Parameter inventory (pin P1, Tables 6-7 l.745-771)."""
     d, f = d_model, ffn_mult * d_model
