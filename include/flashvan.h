@@ -109,6 +109,15 @@ int fv_energy_dense(int32_t B, int32_t N, const int8_t* spins, const float* J, f
 int fv_free_energy(int32_t B, const float* E, const float* logq, double temperature, double* out,
                    void* stream);
 
+/* Replica overlap, Eq. 9: q_b = (1/N) sum_i a_bi c_bi between sample b of one set and sample b of
+ * another (two independent sampling runs, or the two halves of one).
+ *   spins_a, spins_b [device] [B, N] int8 +-1.  dot [device] [B] int32: the exact sum, q_b = dot[b] / N.
+ *   hist [device, may be NULL] N + 1 int32 counters, zeroed by the call: hist[(dot + N) / 2] is the number of
+ *   samples at each of the values -N, -N + 2, ..., N the sum can take, i.e. p(q) = hist / B.  Integer arithmetic
+ *   throughout: bit-exact and order-independent. */
+int fv_overlap(int32_t B, int32_t N, const int8_t* spins_a, const int8_t* spins_b, int32_t* dot, int32_t* hist,
+               void* stream);
+
 void fv_destroy_model(fv_model* m);
 
 /* Build the paper's attention mask from the coupling graph: the ordered Markov boundary of every vertex

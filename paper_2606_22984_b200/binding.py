@@ -17,7 +17,7 @@ _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.s
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
-           "fv_last_error", "fv_markov_mask"]
+           "fv_last_error", "fv_markov_mask", "fv_overlap"]
 
 
 class FvConfig(ctypes.Structure):
@@ -56,6 +56,7 @@ def lib() -> ctypes.CDLL:
         L.fv_kv_bytes.restype = i64
         L.fv_launch_count.restype = i64
         L.fv_last_error.restype = ctypes.c_char_p
+        L.fv_overlap.argtypes = [i32, i32, vp, vp, vp, vp, vp]
         L.fv_markov_mask.argtypes = [i32, i64, vp, vp, i32, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(i32)]
         _lib = L
     return _lib
@@ -181,6 +182,19 @@ def free_energy(E, logq, temperature: float, out=None):
     _check(lib().fv_free_energy(E.numel(), E.data_ptr(), logq.data_ptr(), float(temperature),
                                 res.data_ptr(), _stream()), "fv_free_energy")
     return res
+
+
+def overlap(spins_a, spins_b, want_hist: bool = True):
+    """fv_overlap: (dot int32 [B], hist int32 [N + 1] or None); q = dot / N (Eq. 9)."""
+    a, c = _dev(spins_a, torch.int8), _dev(spins_b, torch.int8)
+    if a.shape != c.shape or a.dim() != 2:
+        raise FlashVanError("overlap: two [B, N] int8 tensors of one shape")
+    B, N = a.shape
+    dot = torch.empty((B,), dtype=torch.int32, device=a.device)
+    hist = torch.empty((N + 1,), dtype=torch.int32, device=a.device) if want_hist else None
+    _check(lib().fv_overlap(B, N, a.data_ptr(), c.data_ptr(), dot.data_ptr(),
+                            hist.data_ptr() if want_hist else None, _stream()), "fv_overlap")
+    return dot, hist
 
 
 def markov_mask(n: int, edge_a, edge_b, position_space: bool = True):

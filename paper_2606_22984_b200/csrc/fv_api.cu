@@ -439,4 +439,14 @@ int fv_free_energy(int32_t B, const float* E, const float* logq, double temperat
     return FV_OK;
 }
 
+int fv_overlap(int32_t B, int32_t N, const int8_t* spins_a, const int8_t* spins_b, int32_t* dot, int32_t* hist,
+               void* stream) {
+    if (!spins_a || !spins_b || !dot) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || N <= 0) return fail(FV_ERR_BAD_ARG, "B and N must be positive");
+    cudaError_t e = fv_launch_overlap(B, N, spins_a, spins_b, dot, hist, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_overlap launch");
+    g_launches++;
+    return FV_OK;
+}
+
 }  // extern "C"

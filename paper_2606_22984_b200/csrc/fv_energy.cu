@@ -257,6 +257,42 @@ cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const floa
     return cudaGetLastError();
 }
 
+// Replica overlap (Eq. 9): dot[b] = sum_i a[b,i] * c[b,i], exact in int32; one warp per sample,
+// 16 spins per lane and load, products and partial sums by dp4a; hist[(dot + N) / 2] += 1 (integer atomics:
+// the result does not depend on their order).
+__global__ void __launch_bounds__(256) overlap_kernel(int B, int N, const int8_t* __restrict__ sa, const int8_t* __restrict__ sc,
+                                                      int32_t* __restrict__ dot, int32_t* __restrict__ hist) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= B) return;
+    const int8_t* a = sa + (size_t)warp * N;
+    const int8_t* c = sc + (size_t)warp * N;
+    int acc = 0;
+    // rows start at arbitrary byte offsets when N is not a multiple of 16: vector loads only if both are aligned
+    const bool vec = ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(c)) & 15) == 0;
+    const int nv = vec ? N / 16 : 0;
+    for (int i = lane; i < nv; i += 32) {
+        const int4 x = __ldg(reinterpret_cast<const int4*>(a) + i), y = __ldg(reinterpret_cast<const int4*>(c) + i);
+        acc = __dp4a(x.x, y.x, acc); acc = __dp4a(x.y, y.y, acc);
+        acc = __dp4a(x.z, y.z, acc); acc = __dp4a(x.w, y.w, acc);
+    }
+    for (int i = nv * 16 + lane; i < N; i += 32) acc += (int)a[i] * (int)c[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) {
+        dot[warp] = acc;
+        if (hist) atomicAdd(hist + ((acc + N) >> 1), 1);
+    }
+}
+
+cudaError_t fv_launch_overlap(int B, int N, const int8_t* sa, const int8_t* sc, int32_t* dot, int32_t* hist, cudaStream_t s) {
+    if (hist) {
+        cudaError_t e = cudaMemsetAsync(hist, 0, sizeof(int32_t) * (size_t)(N + 1), s);
+        if (e != cudaSuccess) return e;
+    }
+    overlap_kernel<<<(B + 7) / 8, 256, 0, s>>>(B, N, sa, sc, dot, hist);
+    return cudaGetLastError();
+}
+
 cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out, cudaStream_t s) {
     free_energy_kernel<<<1, 1024, 0, s>>>(B, E, logq, T, out);
     return cudaGetLastError();

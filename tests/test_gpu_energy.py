@@ -66,3 +66,36 @@ def test_free_energy_reduction():
         mean, std = O.free_energy(E, lq, 1.0 / T)
         got = fv.free_energy(dev(E), dev(lq), T).cpu().numpy()
         assert abs(got[0] - mean) < 1e-9 * abs(mean) and abs(got[1] - std) < 1e-9 * std
+
+
+@pytest.mark.parametrize("B,N", [(1024, 4096), (257, 1000), (33, 17), (5, 1), (64, 16), (3, 4099)])
+def test_overlap_matches_oracle_bit_exact(B, N):
+    """Eq. 9: integer sums and the p(q) histogram, bit-exact (N a multiple of 16 or not: aligned vector path
+    and byte tail; a row offset that breaks the alignment)."""
+    rng = np.random.default_rng(B * 7919 + N)
+    a = (rng.integers(0, 2, size=(B, N)) * 2 - 1).astype(np.int8)
+    c = a.copy()
+    flip = rng.random((B, N)) < rng.random((B, 1))            # per-sample flip rate: the whole range of q
+    c[flip] *= -1
+    dot_o, hist_o = O.overlap(a, c)
+    dot_g, hist_g = fv.overlap(dev(a), dev(c))
+    assert np.array_equal(dot_g.cpu().numpy().astype(np.int64), dot_o)
+    assert np.array_equal(hist_g.cpu().numpy().astype(np.int64), hist_o)
+    dot_g2, none = fv.overlap(dev(a), dev(a), want_hist=False)
+    assert none is None and (dot_g2.cpu().numpy() == N).all()
+
+
+def test_overlap_of_two_sampling_runs():
+    """The paper's use: two independent sampling runs of one model (uniform seeds 1 and 2) -> q per replica pair."""
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=8, n_sites=64)
+    B = 96
+    weights, posemb = W.make_weights(w), W.make_posemb(w)
+    rp, col = W.make_mask_csr(w)
+    model = fv.create_model(w, weights, rp, col, posemb, B)
+    s1 = model.sample(dev(W.make_uniforms(w, B, 1)))[0].clone()
+    s2 = model.sample(dev(W.make_uniforms(w, B, 2)))[0].clone()
+    dot_g, hist_g = fv.overlap(s1, s2)
+    dot_o, hist_o = O.overlap(s1.cpu().numpy(), s2.cpu().numpy())
+    assert np.array_equal(dot_g.cpu().numpy().astype(np.int64), dot_o)
+    assert np.array_equal(hist_g.cpu().numpy().astype(np.int64), hist_o) and int(hist_g.sum()) == B
+    model.close()
