@@ -45,7 +45,7 @@ def check_log_prob(w, model, weights, posemb, rp, col, spins, tol=TOL_P):
     return dp
 
 
-def check_sample(w, model, weights, posemb, rp, col, u, tol=TOL_P):
+def check_sample(w, model, weights, posemb, rp, col, u, tol=TOL_P, chain_tol=2e-4):
     spins_g, lq_g, cp_g = model.sample(dev(u), want_cond_p=True)
     spins_g = spins_g.cpu().numpy()
     cp_g = cp_g.cpu().numpy().astype(np.float64)
@@ -63,8 +63,8 @@ def check_sample(w, model, weights, posemb, rp, col, u, tol=TOL_P):
     assert (np.abs(lq_g - lq_o) <= bound).all()
     # chain rule on the GPU: teacher-forced pass over its own samples reproduces its log q
     lq_tf, cp_tf = model.log_prob(dev(spins_g), want_cond_p=True)
-    assert np.abs(cp_tf.cpu().numpy() - cp_g).max() <= 2e-4
-    assert np.abs(lq_tf.cpu().numpy() - lq_g).max() <= 2e-4 * max(1.0, np.abs(lq_g).max())
+    assert np.abs(cp_tf.cpu().numpy() - cp_g).max() <= chain_tol
+    assert np.abs(lq_tf.cpu().numpy() - lq_g).max() <= chain_tol * max(1.0, np.abs(lq_g).max())
     return int(tie.sum()), int(mism.sum())
 
 
@@ -286,3 +286,42 @@ def test_markov_boundary_mask_from_the_library(periodic):
     check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=3))
     check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=3))
     model.close()
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_seeded_shape_and_mask_scan(seed):
+    """Seeded scan over what the library accepts: d in {32, 64, 128, 256} with every supported head width,
+    1-3 layers, W_O on/off, both LN2 placements, N from 1 to 150, batch sizes around the kernels' group sizes
+    (1, 7, 8, 9, 31, 149, 300, 1185), and full / band / random / self-only masks; sample and log_prob against
+    the fp64 reference, eight draws per seed.  The two GPU paths (sampler; teacher-forced pass, which for d = 256
+    or W_O is the chunked kernel with its own accumulation order) round to bf16 at the same places but from
+    fp32 values that differ in the last bits, so here they are held to 5e-4 of each other (seen: 2.2e-4 at
+    d = 256, three layers, W_O) instead of the 2e-4 the BASELINE configs meet; each is within 2e-3 of the
+    reference either way."""
+    rng = np.random.default_rng(9000 + seed)
+    heads = {32: (16,), 64: (16, 32), 128: (16, 32), 256: (64,)}
+    for case in range(8):
+        d = int(rng.choice([32, 64, 128, 256]))
+        dh = int(rng.choice(heads[d]))
+        N = int(rng.choice([1, 2, 5, 16, 17, 33, 64, 97, 150]))
+        B = int(rng.choice([1, 2, 7, 8, 9, 31, 64, 149, 300, 1185]))
+        kind = str(rng.choice(["full", "band", "random", "selfonly"]))
+        if kind == "full":
+            rows = [np.arange(t + 1) for t in range(N)]
+        elif kind == "band":
+            width = int(rng.integers(1, 40))
+            rows = [np.arange(max(0, t - width), t + 1) for t in range(N)]
+        elif kind == "selfonly":
+            rows = [np.array([t]) for t in range(N)]
+        else:
+            density = rng.random()
+            rows = [np.concatenate([np.nonzero(rng.random(t) < density)[0], [t]]) for t in range(N)]
+        rp = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int32)
+        col = np.concatenate(rows).astype(np.int32)
+        w = dataclasses.replace(W.CONFIGS["cfg3"], L=N, n_sites=N, d_model=d, n_heads=d // dh,
+                                n_layers=int(rng.integers(1, 4)), has_wo=int(rng.random() < 0.25),
+                                ln2_style=int(rng.random() < 0.3))
+        model, weights, posemb, rp, col = build(w, B, mask=(rp, col))
+        check_log_prob(w, model, weights, posemb, rp, col, W.make_spins(w, B, seed=case))
+        check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=case), chain_tol=5e-4)
+        model.close()
