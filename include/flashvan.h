@@ -118,6 +118,19 @@ int fv_free_energy(int32_t B, const float* E, const float* logq, double temperat
 int fv_overlap(int32_t B, int32_t N, const int8_t* spins_a, const int8_t* spins_b, int32_t* dot, int32_t* hist,
                void* stream);
 
+/* Local Monte Carlo refinement of samples (SI I.C l.583-595 "short LMC procedure").  The
+ * paper names neither the acceptance rule nor the number of sweeps; this is the textbook Metropolis single-spin
+ * flip, n_sweeps sweeps over the sites in index order: h_i = sum_j J_ij s_j in the order the adjacency lists the
+ * neighbours (fp32), dE = 2 s_i h_i, flip iff beta * dE < e, e a standard exponential variate (-ln u) supplied
+ * by the caller, so P(accept) = min(1, exp(-beta dE)) and the kernel itself draws nothing.
+ *   spins [device] [B, N] int8 +-1, updated in place.  adj_rowptr / adj_col / adj_val [device]: FULL symmetric
+ *   adjacency CSR (every bond listed at both ends; fv_energy_csr's bond list names each bond once).
+ *   exp_variates [device] [B, n_sweeps, N] fp32 >= 0 (may be NULL when n_sweeps = 0).  accepted [device, may be NULL] [B] int32: flips accepted
+ *   per sample.  N <= 49152 (a sample's spins stay in shared memory for all sweeps).  Bit-reproducible. */
+int fv_lmc_sweeps(int32_t B, int32_t N, int32_t n_sweeps, int8_t* spins, const int32_t* adj_rowptr,
+                  const int32_t* adj_col, const float* adj_val, float beta, const float* exp_variates,
+                  int32_t* accepted, void* stream);
+
 void fv_destroy_model(fv_model* m);
 
 /* Build the paper's attention mask from the coupling graph: the ordered Markov boundary of every vertex

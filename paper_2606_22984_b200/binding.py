@@ -17,7 +17,7 @@ _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.s
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
-           "fv_last_error", "fv_markov_mask", "fv_overlap"]
+           "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps"]
 
 
 class FvConfig(ctypes.Structure):
@@ -56,6 +56,7 @@ def lib() -> ctypes.CDLL:
         L.fv_kv_bytes.restype = i64
         L.fv_launch_count.restype = i64
         L.fv_last_error.restype = ctypes.c_char_p
+        L.fv_lmc_sweeps.argtypes = [i32, i32, i32, vp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
         L.fv_overlap.argtypes = [i32, i32, vp, vp, vp, vp, vp]
         L.fv_markov_mask.argtypes = [i32, i64, vp, vp, i32, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(i32)]
         _lib = L
@@ -182,6 +183,22 @@ def free_energy(E, logq, temperature: float, out=None):
     _check(lib().fv_free_energy(E.numel(), E.data_ptr(), logq.data_ptr(), float(temperature),
                                 res.data_ptr(), _stream()), "fv_free_energy")
     return res
+
+
+def lmc_sweeps(spins, adj_rowptr, adj_col, adj_val, beta: float, exp_variates):
+    """fv_lmc_sweeps: Metropolis sweeps in place on `spins` (int8 CUDA tensor [B, N]); exp_variates fp32
+    [B, n_sweeps, N].  Returns the accepted-flip counts (int32 [B])."""
+    if spins.dtype != torch.int8 or not spins.is_cuda or not spins.is_contiguous() or spins.dim() != 2:
+        raise FlashVanError("lmc_sweeps: spins must be a contiguous int8 CUDA tensor [B, N] (updated in place)")
+    B, N = spins.shape
+    ev = _dev(exp_variates, torch.float32)
+    if ev.dim() != 3 or ev.shape[0] != B or ev.shape[2] != N:
+        raise FlashVanError("lmc_sweeps: exp_variates must be [B, n_sweeps, N]")
+    rp, col, val = _dev(adj_rowptr, torch.int32), _dev(adj_col, torch.int32), _dev(adj_val, torch.float32)
+    acc = torch.empty((B,), dtype=torch.int32, device=spins.device)
+    _check(lib().fv_lmc_sweeps(B, N, ev.shape[1], spins.data_ptr(), rp.data_ptr(), col.data_ptr(), val.data_ptr(),
+                               float(beta), ev.data_ptr(), acc.data_ptr(), _stream()), "fv_lmc_sweeps")
+    return acc
 
 
 def overlap(spins_a, spins_b, want_hist: bool = True):

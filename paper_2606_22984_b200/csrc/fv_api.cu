@@ -449,4 +449,17 @@ int fv_overlap(int32_t B, int32_t N, const int8_t* spins_a, const int8_t* spins_
     return FV_OK;
 }
 
+int fv_lmc_sweeps(int32_t B, int32_t N, int32_t n_sweeps, int8_t* spins, const int32_t* adj_rowptr,
+                  const int32_t* adj_col, const float* adj_val, float beta, const float* exp_variates,
+                  int32_t* accepted, void* stream) {
+    if (B <= 0 || N <= 0 || n_sweeps < 0) return fail(FV_ERR_BAD_ARG, "B, N must be positive and n_sweeps >= 0");
+    if (!spins || !adj_rowptr || !adj_col || !adj_val || (n_sweeps > 0 && !exp_variates)) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (N > 48 * 1024) return fail(FV_ERR_BAD_SHAPE, "fv_lmc_sweeps keeps a sample's spins in shared memory: N <= 49152");
+    cudaError_t e = fv_launch_lmc(B, N, n_sweeps, spins, adj_rowptr, adj_col, adj_val, beta, exp_variates, accepted,
+                                  (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_lmc_sweeps launch");
+    g_launches++;
+    return FV_OK;
+}
+
 }  // extern "C"

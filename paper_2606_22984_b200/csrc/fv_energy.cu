@@ -293,6 +293,57 @@ cudaError_t fv_launch_overlap(int B, int N, const int8_t* sa, const int8_t* sc, 
     return cudaGetLastError();
 }
 
+// Local Monte Carlo refinement (Metropolis single-spin flips in site order, the
+// acceptance test beta * dE < e with a caller-supplied exponential variate e -- no transcendental, so every
+// decision is one fp32 multiplication and one comparison).  A sweep is sequential in the sites, so one warp owns
+// one sample: its spins live in shared memory for all sweeps, lane 0 walks the sites (h_i accumulated in fp32 in
+// adjacency order), the warp loads and stores the row with coalesced 16-byte accesses.
+__global__ void __launch_bounds__(256) lmc_kernel(int B, int N, int n_sweeps, int8_t* __restrict__ spins,
+                                                  const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                                                  const float* __restrict__ val, float beta, const float* __restrict__ ev,
+                                                  int32_t* __restrict__ accepted, int row_stride) {
+    extern __shared__ __align__(16) int8_t lmc_rows[];
+    const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int b = blockIdx.x * (blockDim.x >> 5) + wib;
+    if (b >= B) return;
+    int8_t* s = lmc_rows + (size_t)wib * row_stride;
+    int8_t* g = spins + (size_t)b * N;
+    for (int i = lane; i < N; i += 32) s[i] = g[i];
+    __syncwarp();
+    int acc = 0;
+    if (lane == 0) {
+        const float* e = ev + (size_t)b * n_sweeps * N;
+        for (int k = 0; k < n_sweeps; ++k, e += N) {
+            int p0 = __ldg(rowptr);
+            for (int i = 0; i < N; ++i) {
+                const int p1 = __ldg(rowptr + i + 1);
+                float h = 0.f;
+                for (int p = p0; p < p1; ++p) h = __fadd_rn(h, __fmul_rn(__ldg(val + p), (float)s[__ldg(col + p)]));
+                p0 = p1;
+                const float dE = __fmul_rn(__fmul_rn(2.0f, (float)s[i]), h);
+                if (__fmul_rn(beta, dE) < __ldg(e + i)) {
+                    s[i] = -s[i];
+                    ++acc;
+                }
+            }
+        }
+        if (accepted) accepted[b] = acc;
+    }
+    __syncwarp();
+    for (int i = lane; i < N; i += 32) g[i] = s[i];
+}
+
+cudaError_t fv_launch_lmc(int B, int N, int n_sweeps, int8_t* spins, const int32_t* rowptr, const int32_t* col,
+                          const float* val, float beta, const float* ev, int32_t* accepted, cudaStream_t s) {
+    const int row_stride = (N + 15) / 16 * 16;
+    int warps = 8;
+    while (warps > 1 && (size_t)warps * row_stride > 48 * 1024) warps >>= 1;
+    if ((size_t)warps * row_stride > 48 * 1024) return cudaErrorInvalidValue;
+    lmc_kernel<<<(B + warps - 1) / warps, warps * 32, (size_t)warps * row_stride, s>>>(B, N, n_sweeps, spins, rowptr, col, val,
+                                                                                      beta, ev, accepted, row_stride);
+    return cudaGetLastError();
+}
+
 cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out, cudaStream_t s) {
     free_energy_kernel<<<1, 1024, 0, s>>>(B, E, logq, T, out);
     return cudaGetLastError();

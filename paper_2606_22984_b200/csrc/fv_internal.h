@@ -96,6 +96,9 @@ cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, doub
 cudaError_t fv_launch_overlap(int B, int N, const int8_t* sa, const int8_t* sc, int32_t* dot, int32_t* hist,
                               cudaStream_t s);
 
+cudaError_t fv_launch_lmc(int B, int N, int n_sweeps, int8_t* spins, const int32_t* rowptr, const int32_t* col,
+                          const float* val, float beta, const float* ev, int32_t* accepted, cudaStream_t s);
+
 // fv_mask.cu: rows[i] = ordered Markov boundary of vertex i, ascending; -1 and a
 // message in err on a bad edge.
 int fv_markov_rows(int32_t n, int64_t n_edges, const int32_t* edge_a, const int32_t* edge_b,
