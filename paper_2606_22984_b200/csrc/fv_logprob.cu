@@ -43,7 +43,7 @@ template <int D> struct LpGeo {
     static constexpr int H_BYTES = TM * HC * 2;
     static constexpr int WBUF = W1_BYTES + W2_BYTES;
     static constexpr int FFN_SMEM = A_BYTES + H_BYTES + 2 * WBUF;
-    static constexpr int TMEM_F = (HC + D) <= 256 ? 256 : 512;
+    static constexpr int TMEM_F = (2 * HC + D) <= 256 ? 256 : 512;   // two GEMM 1 accumulators + GEMM 2's
 };
 
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
@@ -87,20 +87,22 @@ __device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __re
 }
 
 // Exact-GELU 0.5 x (1 + erf(x / sqrt 2)) with erf from Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7,
-// far below the bf16 rounding of the result): one rcp.approx, one ex2.approx, six FMAs -- the
-// epilogue of the fused FFN evaluates 4d of these per row and bounds the kernel.
+// far below the bf16 rounding of the result): erf(z) = 1 - (a1 t + .. + a5 t^5) exp(-z^2),
+// t = 1 / (1 + p z), z = |x| / sqrt 2.  Written in y = |x| sqrt(log2(e) / 2), so that
+// exp(-z^2) = 2^(-y y) needs no further scaling: one rcp.approx, one ex2.approx and ten FP32
+// instructions -- the epilogue of the fused FFN evaluates 4d of these per row and bounds the kernel.
 __device__ __forceinline__ float gelu_fast(float x) {
-    const float z = fabsf(x) * 0.70710678118654752f;
-    float t;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.3275911f, z, 1.0f)));
+    const float hx = 0.5f * x;
+    const float y = fabsf(x) * 0.84932180028801904f;           // sqrt(log2(e) / 2)
+    float t, ex;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.27273748f, y, 1.0f)));   // p / sqrt(2) / 0.849..
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(-y * y));
     float p = fmaf(1.061405429f, t, -1.453152027f);
     p = fmaf(p, t, 1.421413741f);
     p = fmaf(p, t, -0.284496736f);
     p = fmaf(p, t, 0.254829592f);
-    float ex;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(-z * z * kLog2e));
-    const float e = fmaf(-p * t, ex, 1.0f);                     // erf(|x| / sqrt 2)
-    return 0.5f * x + 0.5f * fabsf(x) * e;                      // 0.5 x (1 + sign(x) e)
+    const float e = fmaf(-p * t, ex, 1.0f);                    // erf(|x| / sqrt 2)
+    return fmaf(fabsf(hx), e, hx);                             // 0.5 x (1 + sign(x) e)
 }
 
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
@@ -509,11 +511,17 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
 
 // --------------------------------------------------------------------------------- FFN
 // h <- h + W2 gelu(W1 LN2(h) + b1) + b2 for a tile of 128 rows (Alg. 2 l.16 form; ln2_style 1:
-// h <- LN2(h) first, Alg. 1 l.5).  The hidden layer is processed in chunks of HC columns:
-//   acc1 (TMEM cols [0,HC))   = A W1_j^T
+// h <- LN2(h) first, Alg. 1 l.5).  The hidden layer is processed in chunks of HC columns, chunk g
+// (counted over all tiles of the CTA) using accumulator buffer g & 1:
+//   acc1[g&1] (TMEM cols [0,HC) / [HC,2HC)) = A W1_j^T
 //   H_j = bf16(gelu(acc1 + b1_j)) -> shared memory, swizzled K-major (it is GEMM 2's A operand)
-//   acc2 (TMEM cols [HC,HC+D)) += H_j W2_j^T
-// W1_j | W2_j arrive as pre-swizzled images by cp.async.bulk, double buffered.
+//   acc2 (TMEM cols [2HC,2HC+D)) += H_j W2_j^T
+// GEMM 1 of chunk g+1 is issued BEFORE the GELU epilogue of chunk g (the second accumulator buffer
+// makes that legal), GEMM 2 of chunk g right after it: the tensor pipe works under the epilogue
+// and no warp waits for an MMA it has just issued -- the only exposed tensor latency is the tile's
+// first GEMM 1 and its last GEMM 2.  W1_j and W2_j arrive as pre-swizzled images by
+// cp.async.bulk in two rings of two slots each (W1's slot is free once GEMM 1 is done, one chunk
+// earlier than W2's), so every weight copy has a whole chunk time to land.
 template <int D>
 __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_constant__ LpArgs a) {
     using G = LpGeo<D>;
@@ -522,14 +530,15 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
     if (umma::smem_u32(sm) & 1023u) __trap();
     unsigned char* sA = sm;
     unsigned char* sH = sm + G::A_BYTES;
-    unsigned char* sW = sH + G::H_BYTES;           // 2 x (W1_j | W2_j)
+    unsigned char* sW1 = sH + G::H_BYTES;          // 2 x W1_j
+    unsigned char* sW2 = sW1 + 2 * G::W1_BYTES;    // 2 x W2_j
     const uint32_t sA_u32 = umma::smem_u32(sA), sH_u32 = umma::smem_u32(sH);
-    __shared__ uint64_t bar_w[2], bar_m1, bar_m2;
+    __shared__ uint64_t bar_w1[2], bar_w2[2], bar_m1[2], bar_m2;
     __shared__ uint32_t tmem_slot;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        umma::mbar_init(&bar_w[0], 1); umma::mbar_init(&bar_w[1], 1);
-        umma::mbar_init(&bar_m1, 1); umma::mbar_init(&bar_m2, 1);
+        for (int i = 0; i < 2; ++i) { umma::mbar_init(&bar_w1[i], 1); umma::mbar_init(&bar_w2[i], 1); umma::mbar_init(&bar_m1[i], 1); }
+        umma::mbar_init(&bar_m2, 1);
         umma::fence_mbar_init();
     }
     if (warp == 0) umma::tmem_alloc<G::TMEM_F>(&tmem_slot);
@@ -538,37 +547,50 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
     __syncthreads();
     umma::fence_after_sync();
     const uint32_t tmem = tmem_slot;
+    const uint32_t tmem_acc2 = tmem + 2 * G::HC;
     constexpr int E = D / 32;
     const uint32_t idesc1 = umma::make_idesc_bf16(TM, G::HC), idesc2 = umma::make_idesc_bf16(TM, D);
     const long long n_tiles = (a.M + TM - 1) / TM;
     const long long my_tiles = blockIdx.x < n_tiles ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     const long long n_chunks = my_tiles * G::NHC;           // weight chunks this CTA will consume
-    auto issue_w = [&](long long gch) {                      // thread 0: chunk gch -> buffer gch & 1
-        const int j = (int)(gch % G::NHC), buf = (int)(gch & 1);
-        uint64_t* bar = &bar_w[buf];
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(umma::smem_u32(bar)), "r"((uint32_t)G::WBUF) : "memory");
-        const unsigned char* src = a.w_img + (size_t)j * G::WBUF;
-        for (int off = 0; off < G::WBUF; off += 16384) {
-            const uint32_t n = min(16384, G::WBUF - off);
+    auto bulk_in = [&](unsigned char* dst, const unsigned char* src, int bytes, uint64_t* bar) {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(umma::smem_u32(bar)), "r"((uint32_t)bytes) : "memory");
+        for (int off = 0; off < bytes; off += 16384) {
+            const uint32_t n = min(16384, bytes - off);
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                         ::"r"(umma::smem_u32(sW + buf * G::WBUF + off)), "l"(src + off), "r"(n), "r"(umma::smem_u32(bar)) : "memory");
+                         ::"r"(umma::smem_u32(dst + off)), "l"(src + off), "r"(n), "r"(umma::smem_u32(bar)) : "memory");
         }
     };
-    if (tid == 0 && n_chunks > 0) issue_w(0);
-    auto issue_mma1 = [&](unsigned char* w1) {               // thread 0: acc1 = A W1_j^T
-        const uint32_t a0 = umma::smem_u32(sA), b0 = umma::smem_u32(w1);
+    auto issue_w1 = [&](long long c) {                       // thread 0: W1 of chunk c -> slot c & 1
+        bulk_in(sW1 + (int)(c & 1) * G::W1_BYTES, a.w_img + (size_t)(c % G::NHC) * G::WBUF, G::W1_BYTES, &bar_w1[c & 1]);
+    };
+    auto issue_w2 = [&](long long c) {                       // thread 0: W2 of chunk c -> slot c & 1
+        bulk_in(sW2 + (int)(c & 1) * G::W2_BYTES, a.w_img + (size_t)(c % G::NHC) * G::WBUF + G::W1_BYTES, G::W2_BYTES, &bar_w2[c & 1]);
+    };
+    auto issue_mma1 = [&](long long c) {                     // thread 0: acc1[c & 1] = A W1_c^T
+        umma::mbar_wait(&bar_w1[c & 1], (uint32_t)((c >> 1) & 1));
+        umma::fence_after_sync();
+        const uint32_t a0 = umma::smem_u32(sA), b0 = umma::smem_u32(sW1 + (int)(c & 1) * G::W1_BYTES);
+        const uint32_t acc = tmem + (uint32_t)(c & 1) * G::HC;
 #pragma unroll
         for (int kb = 0; kb < G::KB; ++kb)
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks)
-                umma::mma_bf16_ss(tmem, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
+                umma::mma_bf16_ss(acc, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
                                   umma::make_desc_sw128(b0 + kb * (G::HC * 128) + ks * 32), idesc1, (kb | ks) != 0);
-        umma::commit(&bar_m1);
+        umma::commit(&bar_m1[c & 1]);
     };
-    uint32_t ph1 = 0;
-    long long n_m2 = 0;                                      // GEMM 2 commits so far (parity of bar_m2)
-    long long gch = 0;
+    if (tid == 0 && n_chunks > 0) {
+        issue_w1(0); issue_w2(0);
+        if (n_chunks > 1) { issue_w1(1); issue_w2(1); }
+    }
+    long long g = 0;                                         // chunks done so far = index of the next one
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (tid == 0 && tile + gridDim.x < n_tiles) {        // the next tile's rows -> L2 while this one computes
+            const long long r0 = (tile + gridDim.x) * TM;
+            const long long nr = a.M - r0 < TM ? a.M - r0 : TM;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(a.h + r0 * D), "r"((uint32_t)(nr * D * 4)) : "memory");
+        }
         // ---- prologue: LN2 -> bf16 A tile (ln2_style 1: the residual stream becomes LN2(h)) -----
         for (int rb = 0; rb < TM / (FFN_THREADS / 32); rb += RB) {
             float x[RB][E];
@@ -591,86 +613,101 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
         }
         umma::fence_smem_to_async();
         __syncthreads();
-        if (tid == 0) {                                // GEMM 1 of the tile's first chunk
-            umma::mbar_wait(&bar_w[gch & 1], (uint32_t)((gch >> 1) & 1));
-            umma::fence_after_sync();
-            issue_mma1(sW + (gch & 1) * G::WBUF);
-        }
-        for (int j = 0; j < G::NHC; ++j, ++gch) {
-            unsigned char* w2 = sW + (int)(gch & 1) * G::WBUF + G::W1_BYTES;
-            // GEMM 1 of this chunk done; tcgen05 ops of one thread complete in issue order, so the
-            // previous chunk's GEMM 2 is done too: H and the other weight buffer are free
-            // this warp's 32 bias values of the chunk are fetched before the wait, not after it
+        if (tid == 0) issue_mma1(g);                   // GEMM 1 of the tile's first chunk
+        for (int j = 0; j < G::NHC; ++j, ++g) {
+            // GEMM 1 of the next chunk goes into the other accumulator buffer, whose last reader
+            // (the epilogue of chunk g-1) finished before the barrier that closed the previous pass
+            if (tid == 0 && j + 1 < G::NHC) issue_mma1(g + 1);
+            // this warp's first 16 bias values of the chunk are fetched before the wait, not after it
             static_assert(G::HC / 32 == NCG_F, "one 32-column block per warp and chunk");
-            float4 bpre[8];
-            {
-                const float4* b1 = reinterpret_cast<const float4*>(a.bias + j * G::HC + (warp >> 2) * 32);
+            const int cb = warp >> 2;
+            const float4* b1 = reinterpret_cast<const float4*>(a.bias + j * G::HC + cb * 32);
+            float4 bq[4];
 #pragma unroll
-                for (int c = 0; c < 8; ++c) bpre[c] = __ldg(b1 + c);
-            }
-            umma::mbar_wait(&bar_m1, ph1);
-            ph1 ^= 1;
+            for (int c = 0; c < 4; ++c) bq[c] = __ldg(b1 + c);
+            umma::mbar_wait(&bar_m1[g & 1], (uint32_t)((g >> 1) & 1));
             umma::fence_after_sync();
-            if (tid == 0 && gch + 1 < n_chunks) issue_w(gch + 1);
-            // ---- epilogue 1: H_j = bf16(gelu(acc1 + b1_j)), 32 columns per warp -------------------
+            if (tid == 0 && g + 2 < n_chunks) issue_w1(g + 2);   // GEMM 1 of chunk g has read its W1 slot
+            // ---- epilogue 1: H_j = bf16(gelu(acc1 + b1_j)), 32 columns per warp in two halves of
+            // 16 (64 live registers fewer than one 32-column read with its bias: room for the
+            // compiler to interleave the dependent chains of eight elements)
             {
                 const int r = (warp & 3) * 32 + lane;
-#pragma unroll 1
-                for (int cb = (warp >> 2); cb < G::HC / 32; cb += NCG_F) {
-                    float v[32];
-                    umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
+                const uint32_t t0 = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(g & 1) * G::HC + cb * 32;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const float4 ba = bpre[2 * c], bb = bpre[2 * c + 1];
+                for (int hf = 0; hf < 2; ++hf) {
+                    float v[16];
+                    umma::tmem_ld16(t0 + hf * 16, v);
+                    float4 bn[4];
+                    if (hf == 0) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) bn[c] = __ldg(b1 + 4 + c);
+                    }
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        const float4 ba = bq[2 * c], bb = bq[2 * c + 1];
                         uint32_t p[4];
                         p[0] = pack_bf16(gelu_fast(v[c * 8 + 0] + ba.x), gelu_fast(v[c * 8 + 1] + ba.y));
                         p[1] = pack_bf16(gelu_fast(v[c * 8 + 2] + ba.z), gelu_fast(v[c * 8 + 3] + ba.w));
                         p[2] = pack_bf16(gelu_fast(v[c * 8 + 4] + bb.x), gelu_fast(v[c * 8 + 5] + bb.y));
                         p[3] = pack_bf16(gelu_fast(v[c * 8 + 6] + bb.z), gelu_fast(v[c * 8 + 7] + bb.w));
-                        const int col = cb * 32 + c * 8;          // hidden column inside the chunk = K of GEMM 2
+                        // H is GEMM 2's operand: the previous chunk's GEMM 2 (issued one pass ago,
+                        // behind it only this chunk's GEMM 1) must have read it before the first store
+                        if (hf == 0 && c == 0 && j > 0) {
+                            umma::mbar_wait(&bar_m2, (uint32_t)((g - 1) & 1));
+                            umma::fence_after_sync();
+                            if (tid == 0 && g + 1 < n_chunks) issue_w2(g + 1);   // ... and its W2 slot is free
+                        }
+                        const int col = cb * 32 + hf * 16 + c * 8;    // hidden column inside the chunk = K of GEMM 2
                         sts128(sH_u32 + (col >> 6) * (TM * 128) + umma::sw128_chunk(r, (col & 63) >> 3), p[0], p[1], p[2], p[3]);
+                    }
+                    if (hf == 0) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) bq[c] = bn[c];
                     }
                 }
             }
             umma::fence_before_sync();
             umma::fence_smem_to_async();
             __syncthreads();
-            if (tid == 0) {
+            if (tid == 0) {                            // GEMM 2 of this chunk
                 umma::fence_after_sync();
-                const uint32_t h0 = umma::smem_u32(sH), b0 = umma::smem_u32(w2);
+                umma::mbar_wait(&bar_w2[g & 1], (uint32_t)((g >> 1) & 1));
+                const uint32_t h0 = umma::smem_u32(sH), b0 = umma::smem_u32(sW2 + (int)(g & 1) * G::W2_BYTES);
 #pragma unroll
                 for (int kb = 0; kb < G::HC / 64; ++kb)
 #pragma unroll
                     for (int ks = 0; ks < 4; ++ks)
-                        umma::mma_bf16_ss(tmem + G::HC, umma::make_desc_sw128(h0 + kb * (TM * 128) + ks * 32),
+                        umma::mma_bf16_ss(tmem_acc2, umma::make_desc_sw128(h0 + kb * (TM * 128) + ks * 32),
                                           umma::make_desc_sw128(b0 + kb * (D * 128) + ks * 32), idesc2, (j | kb | ks) != 0);
                 umma::commit(&bar_m2);
-                if (j + 1 < G::NHC) {                  // next chunk's GEMM 1 right behind: its latency hides
-                    const long long g1 = gch + 1;      // under this chunk's barrier and the next wait
-                    umma::mbar_wait(&bar_w[g1 & 1], (uint32_t)((g1 >> 1) & 1));
-                    umma::fence_after_sync();
-                    issue_mma1(sW + (g1 & 1) * G::WBUF);
-                }
             }
-            ++n_m2;
         }
-        // ---- epilogue 2: h += acc2 + b2 -------------------------------------------------------
-        umma::mbar_wait(&bar_m2, (uint32_t)((n_m2 - 1) & 1));     // the tile's last GEMM 2
-        umma::fence_after_sync();
+        // ---- epilogue 2: h += acc2 + b2; the rows are requested before the wait for the last GEMM 2
         {
             const int r = (warp & 3) * 32 + lane;
             const long long gi = tile * TM + r;
-            for (int cb = (warp >> 2); cb < D / 32; cb += NCG_F) {
+            float4 hv[8];
+            int cb = warp >> 2;
+            if (gi < a.M && cb < D / 32) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) hv[q] = *reinterpret_cast<const float4*>(a.h + gi * D + cb * 32 + q * 4);
+            }
+            umma::mbar_wait(&bar_m2, (uint32_t)((g - 1) & 1));     // the tile's last GEMM 2
+            umma::fence_after_sync();
+            if (tid == 0 && g + 1 < n_chunks) issue_w2(g + 1);
+            for (; cb < D / 32; cb += NCG_F) {
                 float v[32];
-                umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + G::HC + cb * 32, v);
+                umma::tmem_ld32(tmem_acc2 + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
                 if (gi < a.M) {
                     float* hp = a.h + gi * D + cb * 32;
 #pragma unroll
-                    for (int jj = 0; jj < 32; jj += 4) {
-                        float4 hv = *reinterpret_cast<float4*>(hp + jj);
-                        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias2 + cb * 32 + jj));
-                        hv.x += v[jj] + bb.x; hv.y += v[jj + 1] + bb.y; hv.z += v[jj + 2] + bb.z; hv.w += v[jj + 3] + bb.w;
-                        *reinterpret_cast<float4*>(hp + jj) = hv;
+                    for (int q = 0; q < 8; ++q) {
+                        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias2 + cb * 32 + q * 4));
+                        float4 o = hv[q];
+                        o.x += v[q * 4] + bb.x; o.y += v[q * 4 + 1] + bb.y; o.z += v[q * 4 + 2] + bb.z; o.w += v[q * 4 + 3] + bb.w;
+                        if (cb + NCG_F < D / 32) hv[q] = *reinterpret_cast<const float4*>(hp + NCG_F * 32 + q * 4);
+                        *reinterpret_cast<float4*>(hp + q * 4) = o;
                     }
                 }
             }
