@@ -683,38 +683,72 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
                 umma::commit(&bar_m2);
             }
         }
-        // ---- epilogue 2: h += acc2 + b2; the rows are requested before the wait for the last GEMM 2
+        // ---- epilogue 2: h += acc2 + b2.  A TMEM read gives a thread one ROW (32 columns of it), and
+        // row-per-thread global accesses cost 32 L1 wavefronts per instruction (the kernel's top
+        // unit was the LSU data pipe, 54 %): the accumulator goes through shared memory instead
+        // (the A and H tiles are dead after the last GEMM 2; rows padded by 16 B, conflict-free
+        // both ways) in passes of SW columns, and a warp then adds and stores whole row segments.
+        // The residual rows of the first pass are requested before the wait for the last GEMM 2.
         {
-            const int r = (warp & 3) * 32 + lane;
-            const long long gi = tile * TM + r;
-            float4 hv[8];
-            int cb = warp >> 2;
-            if (gi < a.M && cb < D / 32) {
+            constexpr int SW = D >= 128 ? 64 : 32;          // columns per pass (the staging must fit A|H)
+            constexpr int SROW = SW * 4 + 16;              // padded row stride in bytes
+            constexpr int LPRW = SW / 4;                   // lanes per row segment (float4 each)
+            constexpr int RPI = 32 / LPRW;                 // rows per warp instruction
+            constexpr int RPW = TM / (FFN_THREADS / 32);   // rows per warp
+            constexpr int NI = RPW / RPI;
+            static_assert(TM * SROW <= G::A_BYTES + G::H_BYTES, "staging fits in the dead A|H tiles");
+            const int r = (warp & 3) * 32 + lane;          // phase A: this thread's row
+            const int cbl = warp >> 2;                     //          and 32-column block of the pass
+            const int rB = warp * RPW + lane / LPRW;       // phase B: first row, then += RPI
+            const int cB = (lane % LPRW) * 4;              //          column inside the pass
+            float4 hv[NI];
+            auto load_h = [&](int c0) {
 #pragma unroll
-                for (int q = 0; q < 8; ++q) hv[q] = *reinterpret_cast<const float4*>(a.h + gi * D + cb * 32 + q * 4);
-            }
+                for (int i = 0; i < NI; ++i) {
+                    const long long gi = tile * TM + rB + i * RPI;
+                    if (gi < a.M) hv[i] = *reinterpret_cast<const float4*>(a.h + gi * D + c0 + cB);
+                }
+            };
+            load_h(0);
             umma::mbar_wait(&bar_m2, (uint32_t)((g - 1) & 1));     // the tile's last GEMM 2
             umma::fence_after_sync();
             if (tid == 0 && g + 1 < n_chunks) issue_w2(g + 1);
-            for (; cb < D / 32; cb += NCG_F) {
-                float v[32];
-                umma::tmem_ld32(tmem_acc2 + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
-                if (gi < a.M) {
-                    float* hp = a.h + gi * D + cb * 32;
+#pragma unroll 1
+            for (int c0 = 0; c0 < D; c0 += SW) {
+                if (cbl * 32 < SW) {
+                    float v[32];
+                    umma::tmem_ld32(tmem_acc2 + ((uint32_t)((warp & 3) * 32) << 16) + c0 + cbl * 32, v);
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) {
-                        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias2 + cb * 32 + q * 4));
-                        float4 o = hv[q];
-                        o.x += v[q * 4] + bb.x; o.y += v[q * 4 + 1] + bb.y; o.z += v[q * 4 + 2] + bb.z; o.w += v[q * 4 + 3] + bb.w;
-                        if (cb + NCG_F < D / 32) hv[q] = *reinterpret_cast<const float4*>(hp + NCG_F * 32 + q * 4);
-                        *reinterpret_cast<float4*>(hp + q * 4) = o;
+                    for (int q = 0; q < 8; ++q)
+                        sts128(sA_u32 + r * SROW + (cbl * 32 + q * 4) * 4, __float_as_uint(v[q * 4]), __float_as_uint(v[q * 4 + 1]),
+                               __float_as_uint(v[q * 4 + 2]), __float_as_uint(v[q * 4 + 3]));
+                }
+                __syncthreads();
+                const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias2 + c0 + cB));
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int row = rB + i * RPI;
+                    const long long gi = tile * TM + row;
+                    const float4 t = *reinterpret_cast<const float4*>(sA + row * SROW + cB * 4);
+                    if (gi < a.M) {
+                        float4 o = hv[i];
+                        o.x += t.x + bb.x; o.y += t.y + bb.y; o.z += t.z + bb.z; o.w += t.w + bb.w;
+                        *reinterpret_cast<float4*>(a.h + gi * D + c0 + cB) = o;
                     }
+                }
+                if (c0 + SW < D) {
+                    load_h(c0 + SW);
+                    __syncthreads();
                 }
             }
         }
         umma::fence_before_sync();
         __syncthreads();
         umma::fence_after_sync();
+        if (D < 64) {                                  // the staging overwrote the zero K padding of the A tile
+            for (int i = tid; i < G::A_BYTES / 16; i += FFN_THREADS) reinterpret_cast<uint4*>(sA)[i] = make_uint4(0, 0, 0, 0);
+            __syncthreads();
+        }
     }
     __syncthreads();
     if (warp == 0) umma::tmem_dealloc<G::TMEM_F>(tmem);
