@@ -33,7 +33,9 @@ template <int D> struct LpGeo {
     static constexpr int NQ = 3 * D;                      // QKV output features
     static constexpr int NQ_CH = NQ <= 256 ? NQ : 128;    // columns per MMA
     static constexpr int WQ_BYTES = NQ * KP * 2;
-    static constexpr int QKV_SMEM = 1024 + A_BYTES + WQ_BYTES + 64;
+    static constexpr int STG_STRIDE = 4 * D + 16;         // one staged output row: D fp32 (q) or 2D bf16 (K|V), padded
+    static constexpr int STG_BYTES = TM * STG_STRIDE;
+    static constexpr int QKV_SMEM = 1024 + A_BYTES + WQ_BYTES + STG_BYTES + 64;
     static constexpr int TMEM_Q = NQ <= 128 ? 128 : (NQ <= 256 ? 256 : 512);
     // FFN: hidden 4d in chunks of HC columns
     static constexpr int HC = FV_LP_HC;
@@ -143,7 +145,8 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(lp_raw) + 1023) & ~(uintptr_t)1023);
     unsigned char* sA = sm;
     unsigned char* sW = sm + G::A_BYTES;
-    const uint32_t sA_u32 = umma::smem_u32(sA);
+    unsigned char* sS = sW + G::WQ_BYTES;            // output staging (epilogue)
+    const uint32_t sA_u32 = umma::smem_u32(sA), sS_u32 = umma::smem_u32(sS);
     __shared__ uint64_t bar_w, bar_mma;
     __shared__ uint32_t tmem_slot;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -233,35 +236,57 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
         ph ^= 1;
         umma::fence_after_sync();
         // ---- epilogue: + bias; q -> fp32, k|v -> bf16 KV pool row (Alg. 2's cache layout) ---------
+        // A TMEM read hands a thread one ROW; stored from there every instruction would touch 32
+        // lines.  Two passes through a padded staging tile instead (q as fp32, then K|V as the
+        // bf16 row the pool stores -- both 4d bytes wide): a warp then writes whole rows.
         {
-            const int r = (warp & 3) * 32 + lane;
-            const long long gi = tile * TM + r;
-            const bool ok = gi < a.M;
-            const int b = ok ? (int)(gi / a.N) : 0, t = ok ? (int)(gi % a.N) : 0;
-            float* qrow = a.q + gi * D;
-            __nv_bfloat16* kvrow = a.kv + (((size_t)b * a.NL + a.layer) * a.N + t) * (2 * D);
-            for (int cb = (warp >> 2); cb < G::NQ / 32; cb += NCG) {
-                float v[32];
-                umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
-                if (!ok) continue;
-                const int f0 = cb * 32;
+            constexpr int LPRW = D / 4;                    // lanes per staged row (16 B each)
+            constexpr int RPI = 32 / LPRW;                 // rows per warp instruction
+            constexpr int RPW = TM / (LP_THREADS / 32);    // rows per warp
+            const int r = (warp & 3) * 32 + lane;          // staging: this thread's row
+            const int rB = warp * RPW + lane / LPRW;       // storing: first row, then += RPI
+            const int cB = (lane % LPRW) * 16;             //          byte offset inside the row
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+                const int cb0 = pass == 0 ? 0 : D / 32, cb1 = pass == 0 ? D / 32 : G::NQ / 32;
+                for (int cb = cb0 + (warp >> 2); cb < cb1; cb += NCG) {
+                    float v[32];
+                    umma::tmem_ld32(tmem + ((uint32_t)((warp & 3) * 32) << 16) + cb * 32, v);
+                    const int f0 = cb * 32;
 #pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias + f0 + j));
-                    v[j] += bb.x; v[j + 1] += bb.y; v[j + 2] += bb.z; v[j + 3] += bb.w;
-                }
-                if (f0 < D) {
+                    for (int j = 0; j < 32; j += 4) {
+                        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.bias + f0 + j));
+                        v[j] += bb.x; v[j + 1] += bb.y; v[j + 2] += bb.z; v[j + 3] += bb.w;
+                    }
+                    if (pass == 0) {
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4) *reinterpret_cast<float4*>(qrow + f0 + j) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-                } else {
+                        for (int j = 0; j < 32; j += 4)
+                            sts128(sS_u32 + r * G::STG_STRIDE + (f0 + j) * 4, __float_as_uint(v[j]), __float_as_uint(v[j + 1]),
+                                   __float_as_uint(v[j + 2]), __float_as_uint(v[j + 3]));
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < 32; j += 8) {
-                        uint4 p;
-                        p.x = pack_bf16(v[j], v[j + 1]); p.y = pack_bf16(v[j + 2], v[j + 3]);
-                        p.z = pack_bf16(v[j + 4], v[j + 5]); p.w = pack_bf16(v[j + 6], v[j + 7]);
-                        *reinterpret_cast<uint4*>(kvrow + (f0 - D) + j) = p;
+                        for (int j = 0; j < 32; j += 8)
+                            sts128(sS_u32 + r * G::STG_STRIDE + (f0 - D + j) * 2, pack_bf16(v[j], v[j + 1]), pack_bf16(v[j + 2], v[j + 3]),
+                                   pack_bf16(v[j + 4], v[j + 5]), pack_bf16(v[j + 6], v[j + 7]));
                     }
                 }
+                __syncthreads();
+#pragma unroll
+                for (int i = 0; i < RPW / RPI; ++i) {
+                    const int row = rB + i * RPI;
+                    const long long gi = tile * TM + row;
+                    if (gi < a.M) {
+                        const uint4 val = *reinterpret_cast<const uint4*>(sS + row * G::STG_STRIDE + cB);
+                        unsigned char* dst;
+                        if (pass == 0) dst = reinterpret_cast<unsigned char*>(a.q + gi * D);
+                        else {
+                            const int b = (int)(gi / a.N), t = (int)(gi % a.N);
+                            dst = reinterpret_cast<unsigned char*>(a.kv + (((size_t)b * a.NL + a.layer) * a.N + t) * (2 * D));
+                        }
+                        *reinterpret_cast<uint4*>(dst + cB) = val;
+                    }
+                }
+                if (pass == 0) __syncthreads();            // the staging tile is rewritten by the K|V pass
             }
         }
         umma::fence_before_sync();
