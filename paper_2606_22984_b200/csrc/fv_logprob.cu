@@ -354,12 +354,13 @@ __device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t addr) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
 }
-// (x, y) -> packed bf16 pairs hi and lo with hi + lo = (x, y) to ~16 mantissa bits
+// (x, y) -> packed bf16 pairs hi and lo with hi + lo = (x, y) to ~16 mantissa bits.  The pair is
+// rounded by one packed conversion (F2FP, ALU pipe) and widened again by a shift and a mask: the
+// scalar conversions (F2F) share the quarter-rate XU pipe with the softmax's ex2, which was the
+// attention kernel's busiest pipe.  Same round-to-nearest-even results bit for bit.
 __device__ __forceinline__ void split_bf16(float x, float y, uint32_t& hi, uint32_t& lo) {
-    const __nv_bfloat16 hx = __float2bfloat16_rn(x), hy = __float2bfloat16_rn(y);
-    __nv_bfloat162 h(hx, hy);
-    hi = *reinterpret_cast<uint32_t*>(&h);
-    lo = pack_bf16(x - __bfloat162float(hx), y - __bfloat162float(hy));
+    hi = pack_bf16(x, y);
+    lo = pack_bf16(x - __uint_as_float(hi << 16), y - __uint_as_float(hi & 0xffff0000u));
 }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src) : "memory");
