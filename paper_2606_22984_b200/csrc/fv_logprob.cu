@@ -367,7 +367,7 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_constant__ LpArgs a,
+__global__ void __launch_bounds__(D / 16 * 32, 3) lp_attn_mma_kernel(const __grid_constant__ LpArgs a,
                                                                   const int32_t* __restrict__ blk_uptr,
                                                                   const int32_t* __restrict__ ukeys,
                                                                   const uint16_t* __restrict__ amask, int n_blk) {
@@ -380,13 +380,23 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
     const int n_chunks = (U + ATT_UC - 1) / ATT_UC;
     const unsigned char* kvb = reinterpret_cast<const unsigned char*>(a.kv + ((size_t)b * a.NL + a.layer) * a.N * (2 * D));
     const uint32_t sm0 = umma::smem_u32(att_sm);
+    // a thread copies one 16-byte piece of RPI-spaced rows; the chunk's key positions are all
+    // requested first, so the copies wait for ONE index load, not for one per row
     auto stage = [&](int ch) {
+        constexpr int RPI = NTH / PCS, NIT = ATT_UC / RPI;
         const int k0 = ch * ATT_UC, nk = min(ATT_UC, U - k0);
         const uint32_t dst = sm0 + (ch & 1) * BUF;
-        for (int i = tid; i < nk * PCS; i += NTH) {
-            const int r = i / PCS, pc = i - r * PCS;
-            const int key = __ldg(ukeys + u0 + k0 + r);
-            cp_async16(dst + r * RS + pc * 16, kvb + (size_t)key * (4 * D) + pc * 16);
+        const int r0 = tid / PCS, pc = tid - r0 * PCS;
+        int keys[NIT];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int r = r0 + it * RPI;
+            keys[it] = r < nk ? __ldg(ukeys + u0 + k0 + r) : -1;
+        }
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int r = r0 + it * RPI;
+            if (keys[it] >= 0) cp_async16(dst + r * RS + pc * 16, kvb + (size_t)keys[it] * (4 * D) + pc * 16);
         }
         asm volatile("cp.async.commit_group;\n" ::: "memory");
     };
@@ -425,16 +435,28 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
         __syncthreads();
         const uint32_t buf = sm0 + (ch & 1) * BUF;
         const int nst = (min(ATT_UC, U - ch * ATT_UC)) / 16;
-        for (int st = 0; st < nst; ++st) {
+        // the allow masks of step st + 1 are requested before step st is worked on
+        uint32_t nbits[2][2];
+        auto load_bits = [&](int st) {
             const uint16_t* ms = mk + (size_t)(ch * (ATT_UC / 16) + st) * ATT_BQ;
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                nbits[mt][0] = __ldg(ms + mt * 16 + g);
+                nbits[mt][1] = __ldg(ms + mt * 16 + g + 8);
+            }
+        };
+        if (nst > 0) load_bits(0);
+        for (int st = 0; st < nst; ++st) {
             uint32_t bits[2][2];
             bool any[2];
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                bits[mt][0] = __ldg(ms + mt * 16 + g);
-                bits[mt][1] = __ldg(ms + mt * 16 + g + 8);
-                any[mt] = __any_sync(0xffffffffu, (bits[mt][0] | bits[mt][1]) != 0);
+                bits[mt][0] = nbits[mt][0];
+                bits[mt][1] = nbits[mt][1];
             }
+            if (st + 1 < nst) load_bits(st + 1);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) any[mt] = __any_sync(0xffffffffu, (bits[mt][0] | bits[mt][1]) != 0);
             if (!any[0] && !any[1]) continue;
             uint32_t kf[4], vf[4];
             {
@@ -512,7 +534,18 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
         }
         __syncthreads();                               // buffer (ch & 1) is restaged two chunks later
     }
-    // finalise: h += O / l  (Alg. 2 l.15: residual without W_O)
+    // finalise: h += O / l  (Alg. 2 l.15: residual without W_O); the residual rows are all
+    // requested before the first is used
+    float2 hres[2][2][2];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int t = t0 + mt * 16 + g + hh * 8;
+            const float* hp = a.h + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
+#pragma unroll
+            for (int x = 0; x < 2; ++x) hres[mt][hh][x] = t < a.N ? *reinterpret_cast<const float2*>(hp + x * 8) : make_float2(0.f, 0.f);
+        }
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
@@ -526,7 +559,7 @@ __global__ void __launch_bounds__(D / 16 * 32) lp_attn_mma_kernel(const __grid_c
                 float* hp = a.h + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
-                    float2 hv = *reinterpret_cast<float2*>(hp + x * 8);
+                    float2 hv = hres[mt][hh][x];
                     hv.x += o[mt][x][hh * 2] * inv;
                     hv.y += o[mt][x][hh * 2 + 1] * inv;
                     *reinterpret_cast<float2*>(hp + x * 8) = hv;
