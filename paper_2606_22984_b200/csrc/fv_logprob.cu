@@ -419,6 +419,12 @@ __global__ void __launch_bounds__(D / 16 * 32, 3) lp_attn_mma_kernel(const __gri
             split_bf16(hi.x * qs, hi.y * qs, qa[mt][hh + 2], ql[mt][hh + 2]);
         }
     }
+    // the residual rows this warp updates at the very end: start them towards L2 now
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+        const int t = t0 + mt * 16 + (lane >> 1);          // 16 rows x 2 sectors (the head's 64 B) per m-tile
+        if (t < a.N) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(a.h + ((long long)b * a.N + t) * D + head * 16 + (lane & 1) * 8));
+    }
     float o[2][2][4], mrow[2][2], lrow[2][2];
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt)
