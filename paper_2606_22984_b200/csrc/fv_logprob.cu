@@ -88,6 +88,44 @@ __device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __re
     else { const __nv_bfloat16 v = __float2bfloat16_rn(x[0]); sts16(dst, *reinterpret_cast<const uint16_t*>(&v)); }
 }
 
+// LayerNorm with EIGHT lanes per row (four rows per warp instruction): lane j of a row holds the
+// float4 pieces k * 8 + j, k < D / 32, so a row's 128-byte segments are read whole, the two
+// reductions take three shuffle steps instead of five and serve four rows at once.  x holds the
+// row's values on entry and the normalised values on return.
+template <int D>
+__device__ __forceinline__ void ln8_to_tile(float4 (&x)[D / 32], const float* __restrict__ gam, const float* __restrict__ bet,
+                                            float eps, uint32_t sA, int r, int j) {
+    constexpr int NV = D / 32;
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) s += (x[k].x + x[k].y) + (x[k].z + x[k].w);
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    s += __shfl_xor_sync(0xffffffffu, s, 4);
+    const float mean = s * (1.0f / D);
+    float v = 0.f;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const float a0 = x[k].x - mean, a1 = x[k].y - mean, a2 = x[k].z - mean, a3 = x[k].w - mean;
+        v += (a0 * a0 + a1 * a1) + (a2 * a2 + a3 * a3);
+    }
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    const float rstd = rsqrtf(v * (1.0f / D) + eps);
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        const int f0 = (k * 8 + j) * 4;
+        const float4 g = __ldg(reinterpret_cast<const float4*>(gam + f0)), b = __ldg(reinterpret_cast<const float4*>(bet + f0));
+        x[k].x = (x[k].x - mean) * rstd * g.x + b.x;
+        x[k].y = (x[k].y - mean) * rstd * g.y + b.y;
+        x[k].z = (x[k].z - mean) * rstd * g.z + b.z;
+        x[k].w = (x[k].w - mean) * rstd * g.w + b.w;
+        sts64(sA + (f0 >> 6) * (TM * 128) + umma::sw128_chunk(r, (f0 & 63) >> 3) + (f0 & 7) * 2,
+              pack_bf16(x[k].x, x[k].y), pack_bf16(x[k].z, x[k].w));
+    }
+}
+
 // Exact-GELU 0.5 x (1 + erf(x / sqrt 2)) with erf from Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7,
 // far below the bf16 rounding of the result): erf(z) = 1 - (a1 t + .. + a5 t^5) exp(-z^2),
 // t = 1 / (1 + p z), z = |x| / sqrt 2.  Written in y = |x| sqrt(log2(e) / 2), so that
@@ -657,23 +695,30 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(a.h + r0 * D), "r"((uint32_t)(nr * D * 4)) : "memory");
         }
         // ---- prologue: LN2 -> bf16 A tile (ln2_style 1: the residual stream becomes LN2(h)) -----
-        for (int rb = 0; rb < TM / (FFN_THREADS / 32); rb += RB) {
-            float x[RB][E];
+        {
+            constexpr int NV = D / 32, RPW = TM / (FFN_THREADS / 32);     // a warp's 16 rows, four per pass
+            const int sub = lane >> 3, j = lane & 7;
+            constexpr int PIF = NV >= 4 ? 2 : 4;                          // passes whose loads are in flight together
+#pragma unroll 1
+            for (int p0 = 0; p0 < RPW / 4; p0 += PIF) {
+                float4 x[PIF][NV];
 #pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const long long gi = tile * TM + warp + (rb + u) * (FFN_THREADS / 32);
-                if (gi < a.M) ld_row<E>(a.h + gi * D + lane * E, x[u]);
-                else {
+                for (int ps = 0; ps < PIF; ++ps) {
+                    const long long gi = tile * TM + warp * RPW + (p0 + ps) * 4 + sub;
 #pragma unroll
-                    for (int j = 0; j < E; ++j) x[u][j] = 0.f;
+                    for (int k = 0; k < NV; ++k)
+                        x[ps][k] = gi < a.M ? *reinterpret_cast<const float4*>(a.h + gi * D + (k * 8 + j) * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
-            }
 #pragma unroll
-            for (int u = 0; u < RB; ++u) {
-                const int r = warp + (rb + u) * (FFN_THREADS / 32);
-                const long long gi = tile * TM + r;
-                ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
-                if (a.ln2_style == 1 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
+                for (int ps = 0; ps < PIF; ++ps) {
+                    const int r = warp * RPW + (p0 + ps) * 4 + sub;
+                    const long long gi = tile * TM + r;
+                    ln8_to_tile<D>(x[ps], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, j);
+                    if (a.ln2_style == 1 && gi < a.M) {
+#pragma unroll
+                        for (int k = 0; k < NV; ++k) *reinterpret_cast<float4*>(a.h + gi * D + (k * 8 + j) * 4) = x[ps][k];
+                    }
+                }
             }
         }
         umma::fence_smem_to_async();
