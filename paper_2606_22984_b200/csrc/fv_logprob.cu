@@ -54,39 +54,6 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, ui
 __device__ __forceinline__ void sts64(uint32_t addr, uint32_t x, uint32_t y) {
     asm volatile("st.shared.v2.b32 [%0], {%1,%2};\n" ::"r"(addr), "r"(x), "r"(y) : "memory");
 }
-__device__ __forceinline__ void sts32(uint32_t addr, uint32_t x) {
-    asm volatile("st.shared.b32 [%0], %1;\n" ::"r"(addr), "r"(x) : "memory");
-}
-__device__ __forceinline__ void sts16(uint32_t addr, uint16_t x) {
-    asm volatile("st.shared.b16 [%0], %1;\n" ::"r"(addr), "h"(x) : "memory");
-}
-
-// LayerNorm of one fp32 row (values already in registers, E = D/32 per lane, feature lane*E + j)
-// -> bf16 into the swizzled A tile row `r`.  Returns the normalised values in x (for ln2_style 1).
-template <int D>
-__device__ __forceinline__ void ln_to_tile(float (&x)[D / 32], const float* __restrict__ gam, const float* __restrict__ bet,
-                                           float eps, uint32_t sA, int r, int lane) {
-    constexpr int E = D / 32;
-    float s = 0.f;
-#pragma unroll
-    for (int j = 0; j < E; ++j) s += x[j];
-    const float mean = warp_sum(s) * (1.0f / D);
-    float v = 0.f;
-#pragma unroll
-    for (int j = 0; j < E; ++j) { const float d = x[j] - mean; v += d * d; }
-    const float rstd = rsqrtf(warp_sum(v) * (1.0f / D) + eps);
-#pragma unroll
-    for (int j = 0; j < E; ++j) {
-        const int f = lane * E + j;
-        x[j] = (x[j] - mean) * rstd * __ldg(gam + f) + __ldg(bet + f);
-    }
-    // the lane's E consecutive features sit inside one 16-byte chunk of the swizzled row
-    const int f0 = lane * E;
-    const uint32_t dst = sA + (f0 >> 6) * (TM * 128) + umma::sw128_chunk(r, (f0 & 63) >> 3) + (f0 & 7) * 2;
-    if constexpr (E == 4) sts64(dst, pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]));
-    else if constexpr (E == 2) sts32(dst, pack_bf16(x[0], x[1]));
-    else { const __nv_bfloat16 v = __float2bfloat16_rn(x[0]); sts16(dst, *reinterpret_cast<const uint16_t*>(&v)); }
-}
 
 // LayerNorm with EIGHT lanes per row (four rows per warp instruction): lane j of a row holds the
 // float4 pieces k * 8 + j, k < D / 32, so a row's 128-byte segments are read whole, the two
@@ -147,17 +114,6 @@ __device__ __forceinline__ float gelu_fast(float x) {
 
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
 
-template <int E> __device__ __forceinline__ void ld_row(const float* p, float (&x)[E]) {
-    if constexpr (E == 4) { const float4 v = *reinterpret_cast<const float4*>(p); x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
-    else if constexpr (E == 2) { const float2 v = *reinterpret_cast<const float2*>(p); x[0] = v.x; x[1] = v.y; }
-    else { x[0] = *p; }
-}
-template <int E> __device__ __forceinline__ void st_row(float* p, const float (&x)[E]) {
-    if constexpr (E == 4) *reinterpret_cast<float4*>(p) = make_float4(x[0], x[1], x[2], x[3]);
-    else if constexpr (E == 2) *reinterpret_cast<float2*>(p) = make_float2(x[0], x[1]);
-    else *p = x[0];
-}
-
 struct LpArgs {
     int32_t B, N, NL, layer, d_token, ln2_style;
     float ln_eps;
@@ -207,7 +163,6 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
         for (int i = tid; i < G::A_BYTES / 16; i += LP_THREADS) reinterpret_cast<uint4*>(sA)[i] = make_uint4(0, 0, 0, 0);
         __syncthreads();
     }
-    constexpr int E = D / 32;
     const uint32_t idesc = umma::make_idesc_bf16(TM, G::NQ_CH);
     const long long n_tiles = (a.M + TM - 1) / TM;
     uint32_t ph = 0;
@@ -215,28 +170,37 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     // A warp owns RB = 8 rows of a tile.  Their loads are issued together, and the NEXT tile's rows are
     // requested before this tile's epilogue, so the HBM round trip hides under the MMA and the stores.
     static_assert(TM / (LP_THREADS / 32) == RB, "one load batch per tile");
-    float x[RB][E];
+    // eight lanes per row (see ln8_to_tile): a warp's 8 rows are two passes of four
+    constexpr int NV = D / 32;
+    const int sub = lane >> 3, jl = lane & 7;
+    float4 x[RB / 4][NV];
     auto load_tile = [&](long long tile) {
 #pragma unroll
-        for (int u = 0; u < RB; ++u) {
-            const int r = warp + u * (LP_THREADS / 32);
+        for (int ps = 0; ps < RB / 4; ++ps) {
+            const int r = warp * RB + ps * 4 + sub;
             const long long gi = tile * TM + r;
             if (gi < a.M) {
                 if (a.layer == 0) {                 // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
                     const int t = (int)(gi % a.N);
                     const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
 #pragma unroll
-                    for (int j = 0; j < E; ++j) {
-                        const int f = lane * E + j;
-                        x[u][j] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
-                                                : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
+                    for (int k = 0; k < NV; ++k) {
+                        float e[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const int f = (k * 8 + jl) * 4 + q;
+                            e[q] = f < a.d_token ? __ldg(a.tok_emb + tok * a.d_token + f)
+                                                 : __ldg(a.posemb + (size_t)t * (D - a.d_token) + (f - a.d_token));
+                        }
+                        x[ps][k] = make_float4(e[0], e[1], e[2], e[3]);
                     }
                 } else {
-                    ld_row<E>(a.h + gi * D + lane * E, x[u]);
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) x[ps][k] = *reinterpret_cast<const float4*>(a.h + gi * D + (k * 8 + jl) * 4);
                 }
             } else {
 #pragma unroll
-                for (int j = 0; j < E; ++j) x[u][j] = 0.f;
+                for (int k = 0; k < NV; ++k) x[ps][k] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
     };
@@ -244,11 +208,14 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         // ---- prologue: (embedding) + LN1 -> bf16 A tile ---------------------------------------
 #pragma unroll
-        for (int u = 0; u < RB; ++u) {
-            const int r = warp + u * (LP_THREADS / 32);
+        for (int ps = 0; ps < RB / 4; ++ps) {
+            const int r = warp * RB + ps * 4 + sub;
             const long long gi = tile * TM + r;
-            if (a.layer == 0 && gi < a.M) st_row<E>(a.h + gi * D + lane * E, x[u]);
-            ln_to_tile<D>(x[u], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, lane);
+            if (a.layer == 0 && gi < a.M) {
+#pragma unroll
+                for (int k = 0; k < NV; ++k) *reinterpret_cast<float4*>(a.h + gi * D + (k * 8 + jl) * 4) = x[ps][k];
+            }
+            ln8_to_tile<D>(x[ps], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, jl);
         }
         umma::fence_smem_to_async();
         __syncthreads();
@@ -651,7 +618,6 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
     umma::fence_after_sync();
     const uint32_t tmem = tmem_slot;
     const uint32_t tmem_acc2 = tmem + 2 * G::HC;
-    constexpr int E = D / 32;
     const uint32_t idesc1 = umma::make_idesc_bf16(TM, G::HC), idesc2 = umma::make_idesc_bf16(TM, D);
     const long long n_tiles = (a.M + TM - 1) / TM;
     const long long my_tiles = blockIdx.x < n_tiles ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
