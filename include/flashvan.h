@@ -52,7 +52,6 @@ typedef struct {
     int32_t ln2_style; /* 0: h += FFN(LN2(h)) (Alg. 2 l.346); 1: h = LN2(h); h += FFN(h)      */
                        /*    (Alg. 1 l.237-239); reading A1                                   */
     int32_t max_batch; /* KV pool is sized for this many samples                              */
-    int32_t kv_page;   /* positions per KV page (power of two >= 8); 0 selects 64             */
     float ln_eps;      /* LayerNorm epsilon (reading A6: 1e-5)                                */
 } fv_config;
 
@@ -66,7 +65,9 @@ typedef struct {
  *       row t lists the key positions A(t), ascending, unique, all <= t, last entry == t
  *       (Eq. 3 l.102 sums j <= t; Eq. S1 l.555 is the banded special case).
  *   posemb [host] [N, d_model - d_token] fp32 (Eq. 15).
- * Allocates the paged bf16 KV pool: max_batch * n_layers * N rows of 2d bf16 (K then V), and for
+ * Allocates the bf16 KV pool, a dense array [max_batch][n_layers][N] of rows of 2d bf16 (K then V; every
+ * sample has the same length, so there is no page table), on the CURRENT device -- every later call that
+ * takes the model must be made with that device current (FV_ERR_BAD_ARG otherwise) -- and for
  * d_model <= 128 without W_O the fv_log_prob workspace (two fp32 arrays [max_batch * N, d_model]).
  * Synchronises `stream`.  *out is owned by the library until fv_destroy_model. */
 int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weights,
@@ -104,8 +105,9 @@ int fv_energy_csr(int32_t B, int32_t N, const int8_t* spins, const int32_t* rowp
 int fv_energy_dense(int32_t B, int32_t N, const int8_t* spins, const float* J, float* E,
                     void* stream);
 
-/* Eq. 5: L_b = E_b + T logq_b; out[0] = mean_b L_b, out[1] = population std.
- *   E, logq [device] [B] fp32; out [device] 2 x fp64.  Deterministic single-block fp64 tree. */
+/* Eq. 5: L_b = E_b + T logq_b; out[0] = mean_b L_b, out[1] = population std,
+ *   out[2] = B, out[3] = sum_b (L_b - mean)^2 (the two a batch-sharded run merges across ranks).
+ *   E, logq [device] [B] fp32; out [device] 4 x fp64.  Deterministic single-block fp64 tree. */
 int fv_free_energy(int32_t B, const float* E, const float* logq, double temperature, double* out,
                    void* stream);
 

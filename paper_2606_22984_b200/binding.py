@@ -23,7 +23,7 @@ SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_e
 class FvConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
                 ("n_sites", "n_layers", "d_model", "n_heads", "d_token", "ffn_mult", "has_wo", "act",
-                 "ln2_style", "max_batch", "kv_page")] + [("ln_eps", ctypes.c_float)]
+                 "ln2_style", "max_batch")] + [("ln_eps", ctypes.c_float)]
 
 
 class FlashVanError(RuntimeError):
@@ -78,14 +78,22 @@ def _dev(t: torch.Tensor, dtype) -> torch.Tensor:
     return t
 
 
+def _out(t: torch.Tensor, dtype, shape, like: torch.Tensor) -> torch.Tensor:
+    """A caller-supplied output buffer: same checks as the inputs, plus shape and device."""
+    _dev(t, dtype)
+    if tuple(t.shape) != tuple(shape) or t.device != like.device:
+        raise FlashVanError(f"output buffer must be {tuple(shape)} on {like.device}, got {tuple(t.shape)} on {t.device}")
+    return t
+
+
 def launch_count() -> int:
     return int(lib().fv_launch_count())
 
 
-def make_config(w, max_batch: int, kv_page: int = 64) -> FvConfig:
+def make_config(w, max_batch: int) -> FvConfig:
     """`w` is any object with the Workload fields (n_sites, n_layers, d_model, ...)."""
     return FvConfig(w.n_sites, w.n_layers, w.d_model, w.n_heads, w.d_token, w.ffn_mult, w.has_wo, 0,
-                    w.ln2_style, max_batch, kv_page, float(w.ln_eps))
+                    w.ln2_style, max_batch, float(w.ln_eps))
 
 
 class Model:
@@ -103,6 +111,7 @@ class Model:
         self.cfg = cfg
         self._h = ctypes.c_void_p()
         torch.cuda.init()
+        self.device = torch.device("cuda", torch.cuda.current_device())   # the KV pool lives here
         _check(lib().fv_create_model(ctypes.byref(cfg), weights.ctypes.data, weights.size, rp.ctypes.data,
                                      col.ctypes.data, pe.ctypes.data, _stream(), ctypes.byref(self._h)),
                "fv_create_model")
@@ -115,13 +124,13 @@ class Model:
         """fv_sample: uniforms [B,N] f32 cuda -> (spins int8 [B,N], logq f32 [B], cond_p or None)."""
         u = _dev(uniforms, torch.float32)
         B, N = u.shape
-        if N != self.cfg.n_sites:
-            raise FlashVanError("uniforms must be [B, n_sites]")
+        if N != self.cfg.n_sites or u.device != self.device:
+            raise FlashVanError(f"uniforms must be [B, n_sites] on {self.device}")
         if out is None:
             spins = torch.empty((B, N), dtype=torch.int8, device=u.device)
             logq = torch.empty((B,), dtype=torch.float32, device=u.device)
         else:
-            spins, logq = out
+            spins, logq = _out(out[0], torch.int8, (B, N), u), _out(out[1], torch.float32, (B,), u)
         cp = torch.empty((B, N), dtype=torch.float32, device=u.device) if want_cond_p else None
         _check(lib().fv_sample(self._h, B, u.data_ptr(), spins.data_ptr(), logq.data_ptr(),
                                cp.data_ptr() if cp is not None else None, _stream()), "fv_sample")
@@ -131,9 +140,9 @@ class Model:
         """fv_log_prob: spins int8 [B,N] cuda -> (logq f32 [B], cond_p or None)."""
         s = _dev(spins, torch.int8)
         B, N = s.shape
-        if N != self.cfg.n_sites:
-            raise FlashVanError("spins must be [B, n_sites]")
-        logq = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+        if N != self.cfg.n_sites or s.device != self.device:
+            raise FlashVanError(f"spins must be [B, n_sites] on {self.device}")
+        logq = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else _out(out, torch.float32, (B,), s)
         cp = torch.empty((B, N), dtype=torch.float32, device=s.device) if want_cond_p else None
         _check(lib().fv_log_prob(self._h, B, s.data_ptr(), logq.data_ptr(),
                                  cp.data_ptr() if cp is not None else None, _stream()), "fv_log_prob")
@@ -158,7 +167,7 @@ def create_model(w, weights, mask_rowptr, mask_col, posemb, max_batch: int) -> M
 def energy_csr(spins, rowptr, col, val, integer_couplings: bool, out=None):
     s = _dev(spins, torch.int8)
     B, N = s.shape
-    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else _out(out, torch.float32, (B,), s)
     _check(lib().fv_energy_csr(B, N, s.data_ptr(), _dev(rowptr, torch.int32).data_ptr(),
                                _dev(col, torch.int32).data_ptr(), _dev(val, torch.float32).data_ptr(),
                                1 if integer_couplings else 0, E.data_ptr(), _stream()), "fv_energy_csr")
@@ -171,15 +180,18 @@ def energy_dense(spins, J, out=None):
     J = _dev(J, torch.float32)
     if tuple(J.shape) != (N, N):
         raise FlashVanError("J must be [N, N]")
-    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else out
+    E = torch.empty((B,), dtype=torch.float32, device=s.device) if out is None else _out(out, torch.float32, (B,), s)
     _check(lib().fv_energy_dense(B, N, s.data_ptr(), J.data_ptr(), E.data_ptr(), _stream()), "fv_energy_dense")
     return E
 
 
 def free_energy(E, logq, temperature: float, out=None):
-    """fv_free_energy: returns a 2-element f64 CUDA tensor (mean, std of E + T log q)."""
+    """fv_free_energy: returns a 4-element f64 CUDA tensor (mean, population std of L = E + T log q, count,
+    sum of squared deviations)."""
     E, logq = _dev(E, torch.float32), _dev(logq, torch.float32)
-    res = torch.empty((2,), dtype=torch.float64, device=E.device) if out is None else out
+    if E.shape != logq.shape or E.dim() != 1:
+        raise FlashVanError("free_energy: E and logq must be [B]")
+    res = torch.empty((4,), dtype=torch.float64, device=E.device) if out is None else _out(out, torch.float64, (4,), E)
     _check(lib().fv_free_energy(E.numel(), E.data_ptr(), logq.data_ptr(), float(temperature),
                                 res.data_ptr(), _stream()), "fv_free_energy")
     return res

@@ -33,6 +33,15 @@ int fail(int code, const std::string& msg) {
     return code;
 }
 
+// Every call that takes an fv_model must run on the device the model (its KV pool, its weights) lives on.
+int wrong_device(const fv_model* m) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != m->device)
+        return fail(FV_ERR_BAD_ARG, "the model lives on device " + std::to_string(m->device) + ", the current device is " +
+                                        std::to_string(dev));
+    return 0;
+}
+
 int cuda_fail(cudaError_t e, const char* what) {
     return fail(e == cudaErrorMemoryAllocation ? FV_ERR_OOM : FV_ERR_CUDA,
                 std::string(what) + ": " + cudaGetErrorString(e));
@@ -104,12 +113,13 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     if (!cfg || !weights || !mask_rowptr || !mask_col || !posemb || !out) return fail(FV_ERR_BAD_ARG, "null argument");
     if (!shape_ok(cfg)) return fail(FV_ERR_BAD_SHAPE, "unsupported d_model / n_heads / ffn_mult / act / n_layers");
     if (cfg->max_batch <= 0) return fail(FV_ERR_BAD_ARG, "max_batch must be positive");
-    if (cfg->kv_page != 0 && (cfg->kv_page < 8 || (cfg->kv_page & (cfg->kv_page - 1))))
-        return fail(FV_ERR_BAD_ARG, "kv_page must be 0 or a power of two >= 8");
+    if (!(cfg->ln_eps > 0.f)) return fail(FV_ERR_BAD_ARG, "ln_eps must be positive");
     if (n_weights != n_weights_of(cfg)) return fail(FV_ERR_BAD_SHAPE, "n_weights does not match the configuration");
     const int N = cfg->n_sites, d = cfg->d_model, f = 4 * d, NL = cfg->n_layers;
     // mask validation (reading A11): ascending, unique, 0 <= col <= row, last entry == row
     if (mask_rowptr[0] != 0) return fail(FV_ERR_BAD_MASK, "rowptr[0] != 0");
+    for (int t = 0; t < N; ++t)        // bound every row by rowptr[N] before any mask_col entry is read
+        if (mask_rowptr[t + 1] <= mask_rowptr[t]) return fail(FV_ERR_BAD_MASK, "rowptr not increasing (empty mask row " + std::to_string(t) + ")");
     for (int t = 0; t < N; ++t) {
         const int e0 = mask_rowptr[t], e1 = mask_rowptr[t + 1];
         if (e1 <= e0) return fail(FV_ERR_BAD_MASK, "empty mask row " + std::to_string(t));
@@ -302,10 +312,14 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
 
 void fv_destroy_model(fv_model* m) {
     if (!m) return;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != m->device) cudaSetDevice(m->device);      // free on the model's own device, then restore
     cudaDeviceSynchronize();
     cudaFree(m->dev.kv);
     cudaFree(m->ws);
     cudaFree(m->arena);
+    if (cur >= 0 && cur != m->device) cudaSetDevice(cur);
     delete m;
 }
 
@@ -365,6 +379,7 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
               void* stream) {
     if (!m || !uniforms || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
     if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
+    if (int rc = wrong_device(m)) return rc;
     FvForwardArgs a{};
     a.mode = FV_MODE_SAMPLE;
     a.B = B;
@@ -386,6 +401,7 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {
     if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
     if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
+    if (int rc = wrong_device(m)) return rc;
     const char* force = std::getenv("FLASHVAN_LOGPROB");          // "chunked": the persistent teacher-forcing kernel
     if (!(force && std::strcmp(force, "chunked") == 0)) {
         int n_launch = 0;

@@ -974,12 +974,7 @@ static cudaError_t launch_dec(const FvModelDev& m, const FvForwardArgs& a, int n
     auto kern = fv_decode_kernel<D, DH, NT, CL>;
     using DG = DecGeo<D, NT, CL>;
     const size_t smem = DG::total;
-    static bool attr_set = false;                 // per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DG::total);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    if (cudaError_t e = fv_smem_attr((const void*)kern, (int)DG::total); e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.blockDim = dim3(NTHREADS);
     cfg.dynamicSmemBytes = smem;

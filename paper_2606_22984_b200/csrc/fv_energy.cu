@@ -219,7 +219,8 @@ __global__ void __launch_bounds__(1024) free_energy_kernel(int B, const float* _
         v += d * d;
     }
     const double var = block_reduce<double, 32>(v, red) / B;
-    if (threadIdx.x == 0) { out[0] = mean; out[1] = sqrt(var); }
+    // out[2], out[3]: what a multi-rank merge needs (count and sum of squared deviations, shard.py)
+    if (threadIdx.x == 0) { out[0] = mean; out[1] = sqrt(var); out[2] = (double)B; out[3] = var * B; }
 }
 
 }  // namespace
@@ -241,12 +242,7 @@ cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_
 cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const float* J, float* E, cudaStream_t s) {
     if (N >= 32) {                                  // tensor-core s^T J s (tcgen05, 3-term bf16 split of J)
         const int smem_tc = 65536 + 1024;
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaError_t e = cudaFuncSetAttribute(energy_dense_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_tc);
-            if (e != cudaSuccess) return e;
-            attr_set = true;
-        }
+        if (cudaError_t e = fv_smem_attr((const void*)energy_dense_umma_kernel, smem_tc); e != cudaSuccess) return e;
         energy_dense_umma_kernel<<<(B + 127) / 128, 128, smem_tc, s>>>(B, N, spins, J, E);
         return cudaGetLastError();
     }

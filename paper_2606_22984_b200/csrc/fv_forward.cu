@@ -295,12 +295,7 @@ static cudaError_t launch_one(const FvModelDev& m, const FvForwardArgs& a, int g
     constexpr int NW = 16;
     auto kern = fv_forward_kernel<D, DH, NT, NW>;
     const size_t smem = Geo<D, NT>::total;
-    static bool attr_set = false;                 // per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    if (cudaError_t e = fv_smem_attr((const void*)kern, (int)smem); e != cudaSuccess) return e;
     kern<<<grid, NW * 32, smem, s>>>(m, a);
     return cudaGetLastError();
 }

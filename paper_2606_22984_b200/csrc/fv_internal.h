@@ -4,7 +4,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <map>
+#include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #define FV_MAX_LAYERS 16
@@ -60,6 +63,22 @@ struct FvModelDev {
     float* lp_q;            //                        queries of the current layer, same shape
     FvLayerDev layer[FV_MAX_LAYERS];
 };
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device setting: configure a kernel once per
+// (kernel, device), under a lock (a process may hold models on several GPUs and call from several threads).
+inline cudaError_t fv_smem_attr(const void* kern, int bytes) {
+    static std::mutex mu;
+    static std::map<std::pair<const void*, int>, int> done;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    int& have = done[std::make_pair(kern, dev)];
+    if (have >= bytes) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
 
 enum { FV_MODE_SAMPLE = 0, FV_MODE_LOGPROB = 1 };
 

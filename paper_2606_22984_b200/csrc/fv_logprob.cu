@@ -870,13 +870,11 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
     using G = LpGeo<D>;
     constexpr int att_smem = 2 * ATT_UC * (4 * D + 16);
     static const bool fv_lp_attn_alu = [] { const char* v = std::getenv("FLASHVAN_ATTN"); return v && std::strcmp(v, "alu") == 0; }();
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(lp_qkv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::QKV_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_ffn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::FFN_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_attn_mma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, att_smem);
+    {
+        cudaError_t e = fv_smem_attr((const void*)lp_qkv_kernel<D>, G::QKV_SMEM);
+        if (e == cudaSuccess) e = fv_smem_attr((const void*)lp_ffn_kernel<D>, G::FFN_SMEM);
+        if (e == cudaSuccess) e = fv_smem_attr((const void*)lp_attn_mma_kernel<D>, att_smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     LpArgs a{};
     a.B = B; a.N = m.n_sites; a.NL = m.n_layers; a.d_token = m.d_token; a.ln2_style = m.ln2_style; a.ln_eps = m.ln_eps;

@@ -66,6 +66,11 @@ def test_free_energy_reduction():
         mean, std = O.free_energy(E, lq, 1.0 / T)
         got = fv.free_energy(dev(E), dev(lq), T).cpu().numpy()
         assert abs(got[0] - mean) < 1e-9 * abs(mean) and abs(got[1] - std) < 1e-9 * std
+        assert got[2] == len(E) and abs(got[3] - std * std * len(E)) < 1e-8 * got[3]
+    with pytest.raises(fv.FlashVanError):                              # caller-supplied outputs are validated
+        fv.free_energy(dev(E), dev(lq), 1.0, out=torch.empty(2, dtype=torch.float64, device="cuda"))
+    with pytest.raises(fv.FlashVanError):
+        fv.free_energy(dev(E), dev(lq), 1.0, out=torch.empty(4, dtype=torch.float64))
 
 
 @pytest.mark.parametrize("B,N", [(1024, 4096), (257, 1000), (33, 17), (5, 1), (64, 16), (3, 4099)])

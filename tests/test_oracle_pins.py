@@ -157,6 +157,36 @@ def test_p4_exact_observables_and_kl(cfg1_enum):
     assert abs(mean - Ls.mean()) < 1e-12 and abs(std - Ls.std()) < 1e-12
 
 
+@pytest.mark.parametrize("beta", [0.5, 1.5])
+def test_p4_free_energy_at_beta_not_one(cfg1_enum, beta):
+    """`oracle.free_energy` at the two temperatures cfg3 is evaluated at.  At beta = 1, E + log q / beta and
+    E + beta log q coincide, so only beta != 1 can tell Eq. 5 (F_q = sum_s q [E + ln q / beta])
+    from a beta / T swap.  The exact value comes from the enumerated q and E, not from `free_energy`; the
+    sample estimate must land within 5 sigma of it, and the swapped formula must not (so the pin can fail)."""
+    w, inp, S, lq, E = cfg1_enum
+    q = np.exp(lq)
+    Fq = float((q * (E + lq / beta)).sum())
+    lnZ = float(np.logaddexp.reduce(-beta * E))
+    kl = float((q * (lq - (-beta * E - lnZ))).sum())     # Eq. 4 written out, no F_q in it
+    assert kl >= 0.0 and abs(kl - beta * (Fq - (-lnZ / beta))) < 1e-10
+    spins, lq_s, _ = O.sample(w, inp["weights"], inp["posemb"], inp["mask_rowptr"], inp["mask_col"],
+                              inp["uniforms"])
+    E_s = O.energy_dense(spins, inp["J"])
+    mean, std = O.free_energy(E_s, lq_s, beta)
+    sigma = math.sqrt(float((q * (E + lq / beta - Fq) ** 2).sum()))
+    assert abs(mean - Fq) < 5 * sigma / math.sqrt(len(E_s))
+    swapped = float((q * (E + lq * beta)).sum())         # what a beta <-> T mix-up would converge to
+    assert abs(mean - swapped) > 20 * sigma / math.sqrt(len(E_s))
+    assert abs(std - sigma) < 0.15 * sigma               # spread of L = E + T log q under q, from the enumeration
+
+
+def test_free_energy_std_is_the_population_std():
+    """Two samples with L = 0 and L = 2 at T = 2: mean 1, population std 1 (the ddof = 1 estimate would be
+    sqrt 2).  The GPU kernel and shard.merge_free_energy are held to the same convention."""
+    mean, std = O.free_energy(np.array([0.0, 4.0]), np.array([0.0, -1.0]), 0.5)
+    assert mean == 1.0 and std == 1.0
+
+
 # ----------------------------------------------------------------------- P3: chain rule
 @pytest.mark.parametrize("name", ["cfg1", "ea2d"])
 def test_p3_chain_rule_sample_equals_log_prob(name):

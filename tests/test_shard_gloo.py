@@ -35,8 +35,9 @@ def _worker(rank, world, port, q):
     u = inp["uniforms"][lo:hi]
     spins, lq, _ = O.sample(w, inp["weights"], inp["posemb"], inp["mask_rowptr"], inp["mask_col"], u)
     E = O.energy_csr(spins, inp["bond_rowptr"], inp["bond_col"], inp["bond_val"])
-    mom = shard.local_moments(torch.from_numpy(E), torch.from_numpy(lq), 1.0 / 0.7)
-    mean, std = shard.merge_free_energy(mom)
+    m_r, s_r = O.free_energy(E, lq, 0.7)          # the shard's own reduction (the GPU run takes fv_free_energy's)
+    stats = torch.tensor([m_r, s_r, float(len(E)), s_r * s_r * len(E)], dtype=torch.float64)
+    mean, std = shard.merge_free_energy(stats)
     tmax = shard.max_over_ranks(float(rank + 1))
     q.put((rank, lo, hi, mean, std, tmax))
     dist.destroy_process_group()
