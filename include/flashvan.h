@@ -156,6 +156,19 @@ int fv_markov_mask(int32_t n, int64_t n_edges, const int32_t* edge_a, const int3
 /* Expected n_weights for a configuration (the layout above); < 0 on a bad shape. */
 int64_t fv_n_weights(const fv_config* cfg);
 
+/* Which of the two fv_sample kernels a batch of B samples takes on this model: "chain" (layer-pipelined clusters,
+ * weights resident on chip: d_model = 128, 16-wide heads, no W_O, mask rows of <= 160 entries on average) or
+ * "ring" (one CTA per sample group, weights streamed); "none" for bad arguments.  A static string. */
+const char* fv_sampler_kind(const fv_model* m, int32_t B);
+
+/* Per-kernel device times, for measurement (bench.py's GEMM roofline).  While switched on, the library brackets
+ * the launches of each kernel class with CUDA events on the launching stream.  A call returns, and clears, what
+ * has accumulated since the previous call, then sets the switch to `enable`:
+ *   ms [host, may be NULL] 5 x fp64, launches [host, may be NULL] 5 x int64, in the order
+ *   {fv_sample kernel, fv_log_prob: LN1+QKV GEMM, masked attention, fused LN2+FFN GEMMs, head}.
+ * Synchronises on the recorded events (i.e. on the work they bracket). */
+int fv_profile(int32_t enable, double* ms, int64_t* launches);
+
 /* Bytes of device memory the model's KV pool occupies (0 for NULL). */
 int64_t fv_kv_bytes(const fv_model* m);
 

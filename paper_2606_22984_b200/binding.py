@@ -17,7 +17,7 @@ _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.s
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
-           "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps"]
+           "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps", "fv_profile", "fv_sampler_kind"]
 
 
 class FvConfig(ctypes.Structure):
@@ -58,6 +58,9 @@ def lib() -> ctypes.CDLL:
         L.fv_last_error.restype = ctypes.c_char_p
         L.fv_lmc_sweeps.argtypes = [i32, i32, i32, vp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
         L.fv_overlap.argtypes = [i32, i32, vp, vp, vp, vp, vp]
+        L.fv_profile.argtypes = [i32, vp, vp]
+        L.fv_sampler_kind.argtypes = [vp, i32]
+        L.fv_sampler_kind.restype = ctypes.c_char_p
         L.fv_markov_mask.argtypes = [i32, i64, vp, vp, i32, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(i32)]
         _lib = L
     return _lib
@@ -88,6 +91,16 @@ def _out(t: torch.Tensor, dtype, shape, like: torch.Tensor) -> torch.Tensor:
 
 def launch_count() -> int:
     return int(lib().fv_launch_count())
+
+
+PROFILE_KINDS = ("sample", "lp_qkv", "lp_attn", "lp_ffn", "lp_head")
+
+
+def profile(enable: bool) -> dict:
+    """fv_profile: {kind: (ms, launches)} accumulated since the last call; then switch the timing on or off."""
+    ms, n = (ctypes.c_double * 5)(), (ctypes.c_int64 * 5)()
+    _check(lib().fv_profile(1 if enable else 0, ms, n), "fv_profile")
+    return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(PROFILE_KINDS)}
 
 
 def make_config(w, max_batch: int) -> FvConfig:
@@ -147,6 +160,10 @@ class Model:
         _check(lib().fv_log_prob(self._h, B, s.data_ptr(), logq.data_ptr(),
                                  cp.data_ptr() if cp is not None else None, _stream()), "fv_log_prob")
         return logq, cp
+
+    def sampler_kind(self, B: int) -> str:
+        """Which of the two fv_sample kernels a batch of B takes: "chain" or "ring"."""
+        return lib().fv_sampler_kind(self._h, B).decode()
 
     def close(self):
         if self._h:

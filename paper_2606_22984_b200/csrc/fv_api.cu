@@ -21,12 +21,18 @@ struct fv_model {
     size_t ws_bytes = 0;
     int n_sms = 0;
     int device = 0;
+    double mean_nnz = 0.0;       // mask entries per row
 };
 
 namespace {
 
 thread_local std::string g_err;
 std::atomic<long long> g_launches{0};
+
+// fv_profile: event pairs per kernel class, filled by fv_prof_begin / fv_prof_end while switched on
+std::mutex g_prof_mu;
+bool g_prof_on = false;
+std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof_ev[FV_K_COUNT];
 
 int fail(int code, const std::string& msg) {
     g_err = msg;
@@ -40,6 +46,14 @@ int wrong_device(const fv_model* m) {
         return fail(FV_ERR_BAD_ARG, "the model lives on device " + std::to_string(m->device) + ", the current device is " +
                                         std::to_string(dev));
     return 0;
+}
+
+// fv_sample's choice between its two kernels, before the shape check of the chain sampler.
+bool wants_chain(const fv_model* m) {
+    const char* dmode = std::getenv("FLASHVAN_DECODE");
+    if (dmode && *dmode) return std::strcmp(dmode, "chain") == 0;
+    (void)m;
+    return false;             // opt-in until it beats the streaming kernel
 }
 
 int cuda_fail(cudaError_t e, const char* what) {
@@ -101,7 +115,40 @@ struct Arena {
 
 }  // namespace
 
+void fv_prof_begin(int kind, cudaStream_t s) {
+    std::lock_guard<std::mutex> lock(g_prof_mu);
+    if (!g_prof_on) return;
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+    cudaEventRecord(a, s);
+    g_prof_ev[kind].push_back({a, b});
+}
+void fv_prof_end(int kind, cudaStream_t s) {
+    std::lock_guard<std::mutex> lock(g_prof_mu);
+    if (!g_prof_on || g_prof_ev[kind].empty()) return;
+    cudaEventRecord(g_prof_ev[kind].back().second, s);
+}
+
 extern "C" {
+
+int fv_profile(int32_t enable, double* ms, int64_t* launches) {
+    std::lock_guard<std::mutex> lock(g_prof_mu);
+    for (int k = 0; k < FV_K_COUNT; ++k) {
+        double sum = 0.0;
+        for (auto& pr : g_prof_ev[k]) {
+            float t = 0.f;
+            if (cudaEventSynchronize(pr.second) == cudaSuccess && cudaEventElapsedTime(&t, pr.first, pr.second) == cudaSuccess) sum += t;
+            cudaEventDestroy(pr.first);
+            cudaEventDestroy(pr.second);
+        }
+        if (ms) ms[k] = sum;
+        if (launches) launches[k] = (int64_t)g_prof_ev[k].size();
+        g_prof_ev[k].clear();
+    }
+    (void)cudaGetLastError();
+    g_prof_on = enable != 0;
+    return FV_OK;
+}
 
 const char* fv_last_error(void) { return g_err.c_str(); }
 int64_t fv_launch_count(void) { return g_launches.load(); }
@@ -140,6 +187,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     fv_model* m = new fv_model();
     m->cfg = *cfg;
     m->n_sms = prop.multiProcessorCount;
+    m->mean_nnz = (double)mask_rowptr[N] / N;
     m->device = dev;
     Arena A;
     struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn; };
@@ -387,15 +435,36 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
     sample_geometry(B, m->n_sms, &a.rows_per_group, &nt, &a.n_groups, &grid);
     a.uniforms = uniforms; a.spins_out = spins; a.logq = logq; a.cond_p = cond_p;
     (void)grid;
+    // Two samplers.  Default for d = 128 models with short mask rows (the per-step cost is latency, not KV bytes):
+    // the layer-pipelined clusters of fv_chain.cu with the weights resident in tensor / shared memory; otherwise
+    // (and for every other shape) the streaming kernel of fv_decode.cu.  FLASHVAN_DECODE=chain | ring forces one.
+    const char* dmode = std::getenv("FLASHVAN_DECODE");
+    const bool force_chain = dmode && std::strcmp(dmode, "chain") == 0;
+    if (wants_chain(m)) {
+        fv_prof_begin(FV_K_SAMPLE, (cudaStream_t)stream);
+        cudaError_t ec = fv_launch_chain(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, a, (cudaStream_t)stream);
+        fv_prof_end(FV_K_SAMPLE, (cudaStream_t)stream);
+        if (ec == cudaSuccess) { g_launches++; return FV_OK; }
+        if (ec != cudaErrorNotSupported) return cuda_fail(ec, "fv_sample launch (chain)");
+        (void)cudaGetLastError();
+        if (force_chain) return fail(FV_ERR_BAD_SHAPE, "FLASHVAN_DECODE=chain: shape not covered by the chain sampler");
+    }
     // FLASHVAN_DECODE=cluster opts into the 2-CTA-cluster FFN split (correct, but measured slower than one
     // CTA per sample group on every BASELINE config: DESIGN.md 6.1)
     const char* dm = std::getenv("FLASHVAN_DECODE");
     const int cluster = dm && std::strcmp(dm, "cluster") == 0 && !m->cfg.has_wo;
+    fv_prof_begin(FV_K_SAMPLE, (cudaStream_t)stream);
     cudaError_t e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, m->n_sms, cluster,
                                      (cudaStream_t)stream);
+    fv_prof_end(FV_K_SAMPLE, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "fv_sample launch");
     g_launches++;
     return FV_OK;
+}
+
+const char* fv_sampler_kind(const fv_model* m, int32_t B) {
+    if (!m || B <= 0) return "none";
+    return wants_chain(m) && fv_chain_supported(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B) ? "chain" : "ring";
 }
 
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {

@@ -16,37 +16,13 @@
 // Optional (FLASHVAN_DECODE=cluster): 2-CTA clusters in which each CTA streams only its half of
 // W_1/W_2 and applies it to the rows of both CTAs, exchanging LN2 rows and partial sums through
 // distributed shared memory (correct, measured slower: DESIGN.md 6.1).
-#include "fv_device.cuh"
-
-// Tuning knobs (compile time; the defaults are the measured best).
-#ifndef FV_DEC_ORDER
-#define FV_DEC_ORDER 1      // ring order: 0 = sample-major, 1 = chunk-major
-#endif
-#ifndef FV_DEC_MAXL
-#define FV_DEC_MAXL 8       // 128-bit weight loads in flight per lane in the GEMM phases
-#endif
-#ifndef FV_DEC_WNA
-#define FV_DEC_WNA 0        // 1: weight loads do not allocate in L1
-#endif
-#ifndef FV_DEC_WRING
-#define FV_DEC_WRING 1      // 1: GEMM weights stream through the shared-memory ring (TMA), 0: LDG from L2
-#endif
-#ifndef FV_DEC_KVLSU
-#define FV_DEC_KVLSU 0      // 1: the KV rows are copied by a second producer warp with cp.async (LSU), the weights by TMA
-#endif
-#ifndef FV_DEC_KV_EVICT_FIRST
-#define FV_DEC_KV_EVICT_FIRST 1   // KV rows are read with the L2 evict_first policy
-#endif
-#ifndef FV_DEC_SLOTS
-#define FV_DEC_SLOTS 0      // cap on ring chunks (0 = as many as fit in 227 KB)
-#endif
+#include "fv_ring.cuh"
 
 namespace {
-using namespace fvdev;
+using namespace fvring;
 
-constexpr int NWC = 16;                       // compute warps
-constexpr int NTHREADS = NWC * 32 + (FV_DEC_KVLSU ? 64 : 32);   // + producer warp(s)
-constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
+constexpr int NTHREADS = NWC * 32 + 32;       // compute warps + the producer warp
+constexpr int GEMM_MAXL = 8;                  // 128-bit weight loads in flight per lane when the weights come by LDG (d = 256)
 
 // CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
 template <int D, int NT, bool CL = false>
@@ -67,7 +43,7 @@ struct DecGeo {
     // the residual stream (gemm_ring_kparts: no buffer, 33 KB more ring at 32 rows); with 8 rows the two
     // K-halves go to two warps (measured faster there) and their partial sums reuse the attention-split
     // buffer, which is dead by then
-    static constexpr bool NO_PART = !CL && FV_DEC_WRING && D <= 128 && NT >= 2;
+    static constexpr bool NO_PART = !CL && D <= 128 && NT >= 2;
     static constexpr bool PART_IN_SPLIT = !CL && !NO_PART && G::part_bytes <= split_bytes;
     static constexpr size_t big_bytes = CL ? (qkv_bytes > hid2_bytes + part2_bytes ? qkv_bytes : hid2_bytes + part2_bytes)
                                       : (!(NO_PART || PART_IN_SPLIT)
@@ -83,12 +59,12 @@ struct DecGeo {
     static constexpr int TAB_C = 48, TAB_R = 48;          // per-step copy plan staged in smem (x2: t, t+1)
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
-    static constexpr int NSLOT_CAP = FV_DEC_SLOTS > 0 ? FV_DEC_SLOTS : 60;
+    static constexpr int NSLOT_CAP = 60;
     static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
     static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
     // GEMM weights stream through the same ring (D <= 128): a chunk is CHUNK_BYTES of the packed
     // image = TPCH 16x16 tiles = whole m-tiles (K = D) or one K-part of an m-tile (K = 4D).
-    static constexpr bool WRING = FV_DEC_WRING && D <= 128;
+    static constexpr bool WRING = D <= 128;
     static constexpr int TPCH = CHUNK_BYTES / 512;
     static constexpr int NQ = (3 * D / 16) * (D / 16) / TPCH;     // W_qkv chunks
     static constexpr int NO = (D / 16) * (D / 16) / TPCH;         // W_o
@@ -97,160 +73,6 @@ struct DecGeo {
     static_assert(NSLOT >= 2, "KV ring needs at least two chunks");
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    const uint32_t addr = smem_u32(bar);
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}\n"
-            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-    } while (!done);
-}
-// One bounded probe of a phase (the hardware suspends the thread for a short, implementation-defined time).
-__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
-    uint32_t done;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}\n"
-        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    return done != 0;
-}
-// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier.
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// The same with an L2 eviction policy (createpolicy) attached to the read.
-__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
-}
-// ---- 2-CTA cluster plumbing (distributed shared memory) -------------------------------------
-__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
-}
-__device__ __forceinline__ uint32_t map_to_peer(uint32_t saddr, uint32_t rank) {
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(saddr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void st_peer128(uint32_t raddr, uint4 v) {
-    asm volatile("st.shared::cluster.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(raddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_peer(uint32_t raddr) {
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(raddr) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
-    const uint32_t addr = smem_u32(bar);
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}\n"
-            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWC * 32) : "memory"); }
-__device__ __forceinline__ int ld_acquire_s32(const int* p) {
-    int v;
-    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];\n" : "=r"(v) : "r"(smem_u32(p)) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_release_s32(int* p, int v) {
-    asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
-}
-
-// Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
-// PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
-// with 128-bit shared loads and the matching 16 B of V; RPI = 32/LPR rows per iteration.
-template <int D, int DH, int CH>
-__device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
-                                             float& m, float& l, float (&acc)[8]) {
-    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
-    constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
-    const unsigned char* base = chunk + sub * 16;
-    for (int i0 = 0; i0 < rows; i0 += RPI * U) {
-        uint4 kk[U], vv[U];
-        bool ok[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int row = i0 + u * RPI + rg;
-            ok[u] = row < rows;
-            const unsigned char* p = base + (size_t)(ok[u] ? row : 0) * (4 * D);
-            kk[u] = *reinterpret_cast<const uint4*>(p);
-            vv[u] = *reinterpret_cast<const uint4*>(p + 2 * D);
-        }
-        float s[U];
-        float mx = m;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
-            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
-            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
-            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
-#pragma unroll
-            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-            s[u] = ok[u] ? d : -INFINITY;
-            mx = fmaxf(mx, s[u]);
-        }
-        const float corr = fast_exp2(m - mx);
-        m = mx;
-        l *= corr;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) acc[j] *= corr;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const float p = fast_exp2(s[u] - mx);
-            l += p;
-            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
-            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
-            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
-            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
-        }
-    }
-}
-
-// Consumer side of a ring chunk: wait until the producer has armed this round of the slot (a
-// parity wait can only tell a phase from its predecessor, and another warp may still own the
-// slot's previous round), then wait for the bytes.
-struct RingCtx {
-    unsigned char* ring;
-    uint64_t* bar_full;
-    uint64_t* bar_empty;
-    int* issued;
-};
-template <int NSLOT, int CHUNK_BYTES>
-__device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
-    slot = sq % NSLOT;
-    const uint32_t par = (sq / NSLOT) & 1u;
-    while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
-    mbar_wait(rc.bar_full + slot, par);
-    return rc.ring + (size_t)slot * CHUNK_BYTES;
-}
-__device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
-    // The slot is refilled by cp.async.bulk (async proxy): order this warp's generic-proxy reads of
-    // it before that write.  Without the fence a refill could overtake the reads (seen as run-to-run
-    // differences of ~1e-4 in both samples of a CTA at one step, 15 of 16 fresh-model runs).
-    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-    __syncwarp();
-    if (lane == 0) mbar_arrive(rc.bar_empty + slot);
-}
 
 // GEMM over one tile of 8*NT rows with the weights taken from ring chunks (same contract as
 // gemm_rows).  Chunk j of a matrix holds TPCH consecutive 16x16 tiles of its packed image:
@@ -387,8 +209,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + DG::fixed);
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
-    int* sh_issued = sh_app + 1;                                   // ring chunks armed so far (weights if KVLSU)
-    int* sh_issued_k = FV_DEC_KVLSU ? sh_app + 6 : sh_issued;      // KV chunks armed so far (own producer)
+    int* sh_issued = sh_app + 1;                                   // ring chunks armed so far
     uint64_t* bar_x = reinterpret_cast<uint64_t*>(sh_app + 2);     // [2] cluster exchange barriers (LN2 rows, partials)
     int32_t* tab_c = reinterpret_cast<int32_t*>(smem + DG::fixed + 1024);
     int2* tab_r = reinterpret_cast<int2*>(tab_c + 2 * DG::TAB_C);
@@ -401,7 +222,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
         *sh_app = 0;
         *sh_issued = 0;
-        *sh_issued_k = 0;
         if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
@@ -417,16 +237,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // slot, arm the mbarrier, one bulk copy per run).  VW <= NSLOT, so a lane only ever waits
     // on a chunk issued in an earlier round -- no circular wait with the consumers.
     if (warp >= NWC) {
-        // KVLSU: warp NWC streams the weights by TMA, warp NWC + 1 copies the KV rows with cp.async (a second
-        // copy engine).  Both walk the same chunk sequence; each arms a group only after the other has armed
-        // everything before it, so a slot is never armed more than one round ahead of its barrier.
-        const bool is_tma = warp == NWC, is_lsu = FV_DEC_KVLSU && warp == NWC + 1;
         // The KV rows stream through L2 once per step (one step of the whole batch touches more bytes than L2
         // holds, so none of them survives until its next use): read them evict_first so that they do not push out
         // the GEMM weights every CTA re-reads.  cfg5: 265.6 -> 258.6 ms; a kept (evict_last) fraction of the rows
         // or evict_last on the weights adds nothing.
         uint64_t kv_pol = 0;
-        if (FV_DEC_KV_EVICT_FIRST) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(kv_pol));
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(kv_pol));
         constexpr int VW = NSLOT >= 32 ? 32 : (NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : (NSLOT >= 4 ? 4 : 2)));
         uint32_t seq = 0;
         int it = 0;
@@ -441,12 +257,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         };
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
-            if (!is_tma) {                                   // the KV producer only keeps count
-                seq += (uint32_t)n;
-                if (lane == 0) st_release_s32(sh_issued_k, (int)seq);
-                return;
-            }
-            if (FV_DEC_KVLSU) while ((int)((uint32_t)ld_acquire_s32(sh_issued_k) - seq) < 0) __nanosleep(20);
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
             for (int i0 = 0; i0 < n;) {
                 const int i = i0 + lane;
@@ -491,15 +301,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 return p;
             };
-            const bool kv_mine = FV_DEC_KVLSU ? is_lsu : true;       // this warp copies the KV rows
-            auto count_plan = [&](int t) {                           // chunk count only (the other producer)
-                Plan p{0, 0, 0, nullptr, nullptr};
-                if (t < N) p.nch = __ldg(m.chunk_ptr + t + 1) - __ldg(m.chunk_ptr + t);
-                return p;
-            };
-            Plan cur = kv_mine ? stage_plan(0) : count_plan(0);
+            Plan cur = stage_plan(0);
             for (int t = 0; t < N; ++t) {
-                const Plan nxt = kv_mine ? stage_plan(t + 1) : count_plan(t + 1);
+                const Plan nxt = stage_plan(t + 1);
                 const int nch = cur.nch, nn = cur.nn;
                 const int32_t* cptr = cur.cptr;
                 const int2* rptr = cur.rptr;
@@ -507,69 +311,26 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
                     if (DG::WRING) issue_weights(L.wqkv, DG::NQ);
-                    if (total > 0 && kv_mine) {
+                    if (total > 0) {
                         // rows < t of layer l are complete once step t-1 has appended at layer l
                         const int need = (it * N + (t - 1)) * NL + l + 1;
                         while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
                     }
                     const unsigned char* src_l = reinterpret_cast<const unsigned char*>(
                         m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
-                    if (FV_DEC_KVLSU && is_tma) {
-                        // not mine: all weight chunks before seq + total are armed
-                        if (lane == 0 && total) st_release_s32(sh_issued, (int)(seq + (uint32_t)total));
-                    } else if (is_lsu) {
-                        // ---- cp.async (LSU) copies, one chunk after the other, the whole warp per chunk ----
-                        constexpr int PR = DG::ROW_BYTES / 16;                // 16-byte pieces per row
-                        if (total) while ((int)((uint32_t)ld_acquire_s32(sh_issued) - seq) < 0) __nanosleep(20);
-                        for (int i = 0; i < total; ++i) {
-                            int r, c;
-                            if (FV_DEC_ORDER) {
-                                const int k = i / (GR * nch), rem = i - k * GR * nch;
-                                const int nk = min(GR, n_own - k * GR);
-                                c = rem / nk;
-                                r = k * GR + (rem - c * nk);
-                            } else { r = i / nch; c = i - r * nch; }
-                            const uint32_t sq = seq + (uint32_t)i;
-                            const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
-                            if (lane == 0) mbar_wait(bar_empty + slot, par ^ 1u);
-                            __syncwarp();
-                            const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
-                            const uint32_t dst = smem_u32(ring + (size_t)slot * DG::CHUNK_BYTES);
-                            const int j1 = cptr[c + 1];
-                            for (int j = cptr[c]; j < j1; ++j) {
-                                const int2 run = rptr[j];
-                                const int npc = (run.y & 0xffff) * PR;
-                                const unsigned char* rs = src + (size_t)run.x * DG::ROW_BYTES;
-                                const uint32_t rd = dst + (uint32_t)(run.y >> 16) * DG::ROW_BYTES;
-                                for (int pc = lane; pc < npc; pc += 32)
-                                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(rd + pc * 16), "l"(rs + (size_t)pc * 16) : "memory");
-                            }
-                            // the chunk's full barrier: +1 pending per lane until that lane's copies have landed,
-                            // then the one counted arrival
-                            asm volatile("cp.async.mbarrier.arrive.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar_full + slot)) : "memory");
-                            __syncwarp();
-                            if (lane == 0) {
-                                mbar_arrive(bar_full + slot);
-                                st_release_s32(sh_issued_k, (int)(sq + 1));
-                            }
-                        }
-                    } else
                     for (int i0 = 0; i0 < total;) {
                         const int i = i0 + lane;
                         const uint32_t sq = seq + (uint32_t)i;
                         const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
                         const int npre = ready_prefix(lane < VW && i < total, slot, par);
                         if (lane < npre) {
-                            int r, c;
-                            if (FV_DEC_ORDER) {
-                                // chunk-major inside a round of GR samples (= the samples the compute
-                                // warps work on at the same time), rounds in order: every warp then
-                                // consumes its chunks in ring order
-                                const int k = i / (GR * nch), rem = i - k * GR * nch;
-                                const int nk = min(GR, n_own - k * GR);
-                                c = rem / nk;
-                                r = k * GR + (rem - c * nk);
-                            } else { r = i / nch; c = i - r * nch; }                  // sample-major
+                            // chunk-major inside a round of GR samples (= the samples the compute
+                            // warps work on at the same time), rounds in order: every warp then
+                            // consumes its chunks in ring order
+                            const int k = i / (GR * nch), rem = i - k * GR * nch;
+                            const int nk = min(GR, n_own - k * GR);
+                            const int c = rem / nk;
+                            const int r = k * GR + (rem - c * nk);
                             const int rows = min(CH, nn - c * CH);
                             mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * DG::ROW_BYTES);
                             const unsigned char* src = src_l + (size_t)r * NL * N * DG::ROW_BYTES;
@@ -577,12 +338,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             const int j1 = cptr[c + 1];
                             for (int j = cptr[c]; j < j1; ++j) {
                                 const int2 run = rptr[j];
-                                if (FV_DEC_KV_EVICT_FIRST)
-                                    bulk_g2s_hint(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
-                                                  (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot, kv_pol);
-                                else
-                                    bulk_g2s(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
-                                             (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot);
+                                bulk_g2s_hint(dst + (size_t)(run.y >> 16) * DG::ROW_BYTES, src + (size_t)run.x * DG::ROW_BYTES,
+                                              (uint32_t)(run.y & 0xffff) * DG::ROW_BYTES, bar_full + slot, kv_pol);
                             }
                         }
                         __syncwarp();
@@ -613,8 +370,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     const int rg = lane / LPR, sub = lane % LPR;
     uint32_t seq_base = 0;
     int it = 0;
-    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};          // weight chunks
-    const RingCtx rck{ring, bar_full, bar_empty, sh_issued_k};       // KV chunks (armed by their own producer if KVLSU)
+    const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
     for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
         const int unit = CL ? wu * 2 + (int)crank : wu;
         const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
@@ -663,7 +419,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NQ;
                     } else {
-                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
+                        gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
                     }
                 }
                 cbar();
@@ -706,10 +462,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     }
                     for (int c = sp; c < nch; c += NSPLIT) {
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
-                        const uint32_t sq = seq_base + (uint32_t)(FV_DEC_ORDER ? kr * GR * nch + c * nk + (r - kr * GR)
-                                                                               : r * nch + c);
+                        const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
                         uint32_t slot;
-                        const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rck, sq, slot);
+                        const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
                         attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
                         ring_release(rc, slot, lane);
                     }
@@ -786,7 +541,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NO;
                     } else {
-                        gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
+                        gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
                     }
                 }
                     cbar();
@@ -886,7 +641,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
                             seq_base += DG::N1;
                         } else {
-                            gemm_rows<D / 16, 1, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
+                            gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
                         }
                     }
                     cbar();
@@ -921,7 +676,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
                             seq_base += DG::N2;
                         } else {
-                            gemm_rows<4 * D / 16, KS2, NT, NWC, FV_DEC_MAXL, FV_DEC_WNA != 0>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
+                            gemm_rows<4 * D / 16, KS2, NT, NWC, GEMM_MAXL>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
                         }
                         cbar();
                         for (int i = tid; i < R * D; i += NWC * 32) {
@@ -1007,26 +762,22 @@ static cudaError_t launch_dec_nt(const FvModelDev& m, int nt, const FvForwardArg
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt, const FvForwardArgs& a,
                              int n_sms, int cluster, cudaStream_t s) {
     const int key = d_model * 1000 + d_head;
-    if (cluster && FV_DEC_WRING && d_model <= 128) {
+    if (cluster && d_model <= 128) {
         switch (key) {
-#ifndef FV_DEC_ONLY_128_16
             case 32016: return launch_dec_nt<32, 16, true>(m, nt, a, n_sms, s);
             case 64016: return launch_dec_nt<64, 16, true>(m, nt, a, n_sms, s);
             case 64032: return launch_dec_nt<64, 32, true>(m, nt, a, n_sms, s);
             case 128032: return launch_dec_nt<128, 32, true>(m, nt, a, n_sms, s);
-#endif
             case 128016: return launch_dec_nt<128, 16, true>(m, nt, a, n_sms, s);
             default: break;
         }
     }
     switch (key) {
-#ifndef FV_DEC_ONLY_128_16
         case 32016: return launch_dec_nt<32, 16, false>(m, nt, a, n_sms, s);
         case 64016: return launch_dec_nt<64, 16, false>(m, nt, a, n_sms, s);
         case 64032: return launch_dec_nt<64, 32, false>(m, nt, a, n_sms, s);
         case 128032: return launch_dec_nt<128, 32, false>(m, nt, a, n_sms, s);
         case 256064: return launch_dec_nt<256, 64, false>(m, nt, a, n_sms, s);
-#endif
         case 128016: return launch_dec_nt<128, 16, false>(m, nt, a, n_sms, s);
         default: return cudaErrorInvalidValue;
     }

@@ -21,14 +21,6 @@ __device__ __forceinline__ void mma_bf16(float (&c)[4], const uint4& a, uint32_t
 
 // Weights are immutable for the kernel's lifetime: read-only path, keep in L1/L2.
 __device__ __forceinline__ uint4 ldg_w(const uint4* p) { return __ldg(p); }
-// Streaming variant: no L1 allocation (nothing is reused by this SM within a phase).
-__device__ __forceinline__ uint4 ldg_w_na(const uint4* p) {
-    uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];\n"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
-}
-
 // KV rows are written by this CTA earlier in the same kernel: coherent (non-.nc) load.
 __device__ __forceinline__ uint4 ld_kv(const void* p) {
     uint4 r;
@@ -89,7 +81,7 @@ struct Geo {
 // The weight stream comes from L2 (latency ~1 us under load) and nothing is reused, so the
 // loads of up to TPB tasks (MAXL x 128-bit per lane) are issued before the first MMA: one L2
 // round trip per GEMM phase instead of one per task.
-template <int KT_TOTAL, int KSPLIT, int NT, int NW, int MAXL = 16, bool NA = false, class Epi>
+template <int KT_TOTAL, int KSPLIT, int NT, int NW, int MAXL = 16, class Epi>
 __device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, const __nv_bfloat16* act, int as,
                                           int warp, int lane, Epi epi) {
     constexpr int KT = KT_TOTAL / KSPLIT;
@@ -106,7 +98,7 @@ __device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, 
                 const int mt = task / KSPLIT, ks = task - mt * KSPLIT;
                 const uint4* w = wp + ((size_t)mt * KT_TOTAL + ks * KT) * 32 + lane;
 #pragma unroll
-                for (int u = 0; u < KU; ++u) a[tb][u] = NA ? ldg_w_na(w + u * 32) : ldg_w(w + u * 32);
+                for (int u = 0; u < KU; ++u) a[tb][u] = ldg_w(w + u * 32);
             }
         }
 #pragma unroll
@@ -123,7 +115,7 @@ __device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, 
                 for (int k0 = 0; k0 < KT; k0 += KU) {
                     if (k0 > 0) {
 #pragma unroll
-                        for (int u = 0; u < KU; ++u) a[tb][u] = NA ? ldg_w_na(w + (k0 + u) * 32) : ldg_w(w + (k0 + u) * 32);
+                        for (int u = 0; u < KU; ++u) a[tb][u] = ldg_w(w + (k0 + u) * 32);
                     }
 #pragma unroll
                     for (int u = 0; u < KU; ++u) {

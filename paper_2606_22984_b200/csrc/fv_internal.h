@@ -80,6 +80,12 @@ inline cudaError_t fv_smem_attr(const void* kern, int bytes) {
     return e;
 }
 
+// Optional per-kernel timing (fv_profile in flashvan.h): CUDA events around the launches of one kernel class,
+// recorded on the launching stream; no-ops unless switched on.
+enum { FV_K_SAMPLE = 0, FV_K_LP_QKV = 1, FV_K_LP_ATTN = 2, FV_K_LP_FFN = 3, FV_K_LP_HEAD = 4, FV_K_COUNT = 5 };
+void fv_prof_begin(int kind, cudaStream_t s);
+void fv_prof_end(int kind, cudaStream_t s);
+
 enum { FV_MODE_SAMPLE = 0, FV_MODE_LOGPROB = 1 };
 
 struct FvForwardArgs {
@@ -101,6 +107,8 @@ cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int 
 size_t fv_forward_smem_bytes(int d_model, int nt);
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt,
                              const FvForwardArgs& a, int n_sms, int cluster, cudaStream_t s);
+bool fv_chain_supported(const FvModelDev& m, int d_model, int d_head, int B);
+cudaError_t fv_launch_chain(const FvModelDev& m, int d_model, int d_head, const FvForwardArgs& a, cudaStream_t s);
 cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
                                  float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s);
 void fv_pack_sw128(const float* W, int rows, int K, int ld, int KP, uint16_t* dst);

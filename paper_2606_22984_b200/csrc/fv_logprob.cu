@@ -888,7 +888,10 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
         const FvLayerDev& L = m.layer[l];
         a.layer = l;
         a.w_img = L.img_qkv; a.bias = L.bqkv; a.bias2 = nullptr; a.ln_g = L.ln1_g; a.ln_b = L.ln1_b;
+        fv_prof_begin(FV_K_LP_QKV, s);
         lp_qkv_kernel<D><<<grid, LP_THREADS, G::QKV_SMEM, s>>>(a);
+        fv_prof_end(FV_K_LP_QKV, s);
+        fv_prof_begin(FV_K_LP_ATTN, s);
         if (DH == 16 && m.att_nblk > 0 && !fv_lp_attn_alu) {
             lp_attn_mma_kernel<D><<<(unsigned)(B * m.att_nblk), D / 16 * 32, att_smem, s>>>(a, m.att_blk_uptr, m.att_ukeys,
                                                                                            m.att_mask, m.att_nblk);
@@ -896,10 +899,15 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
             lp_attn_kernel<D, DH><<<(unsigned)((a.M + rows_per_cta - 1) / rows_per_cta), 512, 0, s>>>(a, m.mask_rowptr, m.mask_col,
                                                                                                 rows_per_cta);
         }
+        fv_prof_end(FV_K_LP_ATTN, s);
         a.w_img = L.img_ffn; a.bias = L.b1; a.bias2 = L.b2; a.ln_g = L.ln2_g; a.ln_b = L.ln2_b;
+        fv_prof_begin(FV_K_LP_FFN, s);
         lp_ffn_kernel<D><<<grid_ffn, FFN_THREADS, G::FFN_SMEM, s>>>(a);
+        fv_prof_end(FV_K_LP_FFN, s);
     }
+    fv_prof_begin(FV_K_LP_HEAD, s);
     lp_head_kernel<D><<<B, 256, 0, s>>>(a, m.head_wd, m.head_bd, logq, cond_p);
+    fv_prof_end(FV_K_LP_HEAD, s);
     return cudaGetLastError();
 }
 

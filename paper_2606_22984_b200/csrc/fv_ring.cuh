@@ -1,0 +1,180 @@
+// fv_ring.cuh -- pieces shared by the two samplers of fv_sample (fv_decode.cu: one CTA owns its samples for
+// all layers, weights streamed; fv_chain.cu: a cluster of n_layers CTAs, one layer's weights resident per CTA):
+// mbarrier / TMA bulk-copy / cluster (distributed shared memory) wrappers, the shared-memory KV ring protocol
+// (producer arms chunks in order, one consumer warp per chunk) and the online-softmax update of one query row
+// with the rows of one ring chunk (Eq. 3).
+#pragma once
+#include "fv_device.cuh"
+
+namespace fvring {
+using namespace fvdev;
+
+constexpr int NWC = 16;                       // compute warps of both sampler kernels
+constexpr size_t SMEM_MAX = 232448;           // 227 KB per CTA on sm_100
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!done);
+}
+// One bounded probe of a phase (the hardware suspends the thread for a short, implementation-defined time).
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return done != 0;
+}
+// Non-blocking probe (mbarrier.test_wait never suspends the thread).
+__device__ __forceinline__ bool mbar_test_nb(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return done != 0;
+}
+// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// The same with an L2 eviction policy (createpolicy) attached to the read.
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+// ---- 2-CTA cluster plumbing (distributed shared memory) -------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ uint32_t map_to_peer(uint32_t saddr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_peer128(uint32_t raddr, uint4 v) {
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1,%2,%3,%4};\n" ::"r"(raddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_peer(uint32_t raddr) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(raddr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}\n"
+            : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void cbar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWC * 32) : "memory"); }
+__device__ __forceinline__ int ld_acquire_s32(const int* p) {
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];\n" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_s32(int* p, int v) {
+    asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+
+// Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
+// PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
+// with 128-bit shared loads and the matching 16 B of V; RPI = 32/LPR rows per iteration.
+template <int D, int DH, int CH>
+__device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
+                                             float& m, float& l, float (&acc)[8]) {
+    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
+    constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
+    const unsigned char* base = chunk + sub * 16;
+    for (int i0 = 0; i0 < rows; i0 += RPI * U) {
+        uint4 kk[U], vv[U];
+        bool ok[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int row = i0 + u * RPI + rg;
+            ok[u] = row < rows;
+            const unsigned char* p = base + (size_t)(ok[u] ? row : 0) * (4 * D);
+            kk[u] = *reinterpret_cast<const uint4*>(p);
+            vv[u] = *reinterpret_cast<const uint4*>(p + 2 * D);
+        }
+        float s[U];
+        float mx = m;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
+            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
+            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
+            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
+#pragma unroll
+            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+            s[u] = ok[u] ? d : -INFINITY;
+            mx = fmaxf(mx, s[u]);
+        }
+        const float corr = fast_exp2(m - mx);
+        m = mx;
+        l *= corr;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[j] *= corr;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const float p = fast_exp2(s[u] - mx);
+            l += p;
+            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
+            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
+            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
+            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
+        }
+    }
+}
+
+// Consumer side of a ring chunk: wait until the producer has armed this round of the slot (a
+// parity wait can only tell a phase from its predecessor, and another warp may still own the
+// slot's previous round), then wait for the bytes.
+struct RingCtx {
+    unsigned char* ring;
+    uint64_t* bar_full;
+    uint64_t* bar_empty;
+    int* issued;
+};
+template <int NSLOT, int CHUNK_BYTES>
+__device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
+    slot = sq % NSLOT;
+    const uint32_t par = (sq / NSLOT) & 1u;
+    while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
+    mbar_wait(rc.bar_full + slot, par);
+    return rc.ring + (size_t)slot * CHUNK_BYTES;
+}
+__device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
+    // The slot is refilled by cp.async.bulk (async proxy): order this warp's generic-proxy reads of
+    // it before that write.  Without the fence a refill could overtake the reads (seen as run-to-run
+    // differences of ~1e-4 in both samples of a CTA at one step, 15 of 16 fresh-model runs).
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    __syncwarp();
+    if (lane == 0) mbar_arrive(rc.bar_empty + slot);
+}
+
+}  // namespace fvring
