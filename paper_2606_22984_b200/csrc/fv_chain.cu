@@ -34,12 +34,6 @@ constexpr int CH = fv_ring_ch(D);             // KV rows per ring chunk (host pl
 constexpr int ROW_BYTES = 4 * D, CHUNK_BYTES = CH * ROW_BYTES;
 constexpr int LPR = D / 8, LPH = DH / 8;
 constexpr int TAB_C = 48, TAB_R = 48;
-// KV rows reach the attention warps by (1) TMA copies into the shared-memory ring, or (0) direct 128-bit loads of
-// rows the producer warp has prefetched into L2 one slot ahead (measured: the 8-slot ring that fits next to W_2
-// turns over once per 4000 cycles, whatever the memory latency)
-#ifndef FV_CHAIN_RING
-#define FV_CHAIN_RING 0
-#endif
 // tensor memory columns
 constexpr uint32_t TC_WQKV = 0, TC_W1 = 192, TC_ACC = 448;
 
@@ -170,75 +164,6 @@ __device__ __forceinline__ void ln_row_btile(float* hrow, const float* __restric
     if (replace) *reinterpret_cast<float4*>(hrow + lane * 4) = make_float4(y0, y1, y2, y3);
 }
 
-// Masked attention of one query row straight from the KV pool (Eq. 3): the NSPLIT warps of a row
-// take batches of 8 mask entries in turn; lane layout as attend_chunk (16 lanes cover K of one row with 128-bit
-// loads and fetch the matching 16 B of V, two rows per instruction), the loads of the next batch are in flight
-// while this one is reduced.  `cols` = the row's key positions without its last entry (the step itself).
-template <int NSPLIT>
-__device__ __forceinline__ void attend_gather(const float (&q)[8], const unsigned char* kv_sl, const int32_t* __restrict__ cols,
-                                              int nn, int sp, int rg, int sub, float& m, float& l, float (&acc)[8]) {
-    constexpr int RPI = 32 / LPR, U = 4, BR = RPI * U;
-    const unsigned char* base = kv_sl + sub * 16;
-    const int nb = (nn + BR - 1) / BR;
-    uint4 ka[U], va[U], kb[U], vb[U];
-    auto load = [&](uint4 (&kk)[U], uint4 (&vv)[U], int b) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int e = b * BR + u * RPI + rg;
-#ifdef FV_CHAIN_EXP_SAMEADDR
-            const int pos = __ldg(cols + (e < nn ? e : 0)) & 15;
-#else
-            const int pos = __ldg(cols + (e < nn ? e : 0));
-#endif
-            const unsigned char* p = base + (size_t)pos * ROW_BYTES;
-            kk[u] = ld_kv(p);
-            vv[u] = ld_kv(p + 2 * D);
-        }
-    };
-    auto reduce = [&](const uint4 (&kk)[U], const uint4 (&vv)[U], int b) {
-        float s[U];
-        float mx = m;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
-            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
-            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
-            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
-#pragma unroll
-            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-            s[u] = (b * BR + u * RPI + rg < nn) ? d : -INFINITY;
-            mx = fmaxf(mx, s[u]);
-        }
-        const float corr = fast_exp2(m - mx);
-        m = mx;
-        l *= corr;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) acc[j] *= corr;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const float p = fast_exp2(s[u] - mx);
-            l += p;
-            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
-            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
-            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
-            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
-        }
-    };
-    int b = sp;
-    if (b < nb) load(ka, va, b);
-    while (b < nb) {
-        const int b2 = b + NSPLIT;
-        if (b2 < nb) load(kb, vb, b2);
-        reduce(ka, va, b);
-        b = b2;
-        if (b >= nb) break;
-        const int b3 = b + NSPLIT;
-        if (b3 < nb) load(ka, va, b3);
-        reduce(kb, vb, b);
-        b = b3;
-    }
-}
-
 template <int RMAX>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ ChainArgs a) {
@@ -306,14 +231,15 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
     // did MBc slots earlier, so the stream runs ahead across micro-batch boundaries.
     if (warp >= NWC) {
         if (lane == 0) {                                      // the layer's W_2 image: 8 K-blocks of [128 x 64] bf16
-            mbar_arrive_expect_tx(bar_w, 131072u);
+            constexpr int NKB = 8;
+            mbar_arrive_expect_tx(bar_w, NKB * 16384u);
             const size_t per = ((size_t)FV_LP_HC * D + (size_t)D * FV_LP_HC) * 2;
-            for (int j = 0; j < 8; ++j)
+            for (int j = 0; j < NKB; ++j)
                 bulk_g2s(sh_w2 + j * 16384, L.img_ffn + j * per + (size_t)FV_LP_HC * D * 2, 16384u, bar_w);
         }
         uint64_t kv_pol = 0;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(kv_pol));
-        constexpr int VW = NSLOT >= 8 ? 8 : 4;
+        constexpr int VW = NSLOT >= 16 ? 16 : (NSLOT >= 8 ? 8 : 4);
         uint32_t seq = 0;
         auto ready_prefix = [&](bool active, uint32_t slot, uint32_t par) {
             const bool ok = active && mbar_test_nb(bar_empty + slot, par ^ 1u);
@@ -342,32 +268,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             return p;
         };
-        // The ring is small (W_2 takes 128 KB of the shared memory), so its refill rate is bytes-in-flight over latency.
-        // One slot ahead, the rows a slot will need are therefore pulled into L2 (cp.async.bulk.prefetch.L2, one
-        // request per run of consecutive positions and sample): the ring's copies then pay L2 latency, not HBM's.
-        auto prefetch_slot = [&](int t2, int mb2) {
-            if (t2 >= N) return;
-            const int e0 = __ldg(m.mask_rowptr + t2), nn2 = __ldg(m.mask_rowptr + t2 + 1) - 1 - e0;
-            const int b2 = (g0 + mb2) * a.R, n2 = min(a.R, a.B - b2);
-            if (nn2 <= 0 || ld_acquire_s32(sh_app) < (t2 - 1) * MBc + mb2 + 1) return;     // not appended yet: skip
-            const unsigned char* src2 = reinterpret_cast<const unsigned char*>(m.kv + ((size_t)b2 * NL + l) * N * (2 * D));
-            for (int base = 0; base < nn2; base += 32) {
-                const int e = base + lane;
-                const bool in = e < nn2;
-                const int pos = in ? __ldg(m.mask_col + e0 + e) : -2;
-                const int prev = __shfl_up_sync(0xffffffffu, pos, 1);
-                const bool start = in && (lane == 0 || pos != prev + 1);
-                const unsigned sm = __ballot_sync(0xffffffffu, start), im = __ballot_sync(0xffffffffu, in);
-                if (start) {
-                    const unsigned later = sm & ~((2u << lane) - 1u);
-                    const int len = (later ? __ffs(later) - 1 : __popc(im)) - lane;
-                    for (int r = 0; r < n2; ++r)
-                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n"
-                                     ::"l"(src2 + (size_t)r * NL * N * ROW_BYTES + (size_t)pos * ROW_BYTES), "r"(len * ROW_BYTES) : "memory");
-                }
-                __syncwarp();
-            }
-        };
         Plan cur = stage_plan(0);
         for (int t = 0; t < N; ++t) {
             // the plan of step t + 1 may only replace the table of step t - 1 once every copy of step t - 1 has
@@ -377,12 +277,11 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             for (int mb = 0; mb < MBc; ++mb) {
                 const int b_first = (g0 + mb) * a.R;
                 const int n_own = min(a.R, a.B - b_first);
-                const int total = FV_CHAIN_RING ? n_own * nch : 0;
-                if (n_own * nch > 0) {
+                const int total = n_own * nch;
+                if (total > 0) {
                     const int need = (t - 1) * MBc + mb + 1;
                     while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
                 }
-                if (mb + 1 < MBc) prefetch_slot(t, mb + 1); else prefetch_slot(t + 1, 0);
                 const unsigned char* src_l = reinterpret_cast<const unsigned char*>(m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
                 for (int i0 = 0; i0 < total;) {
                     const int i = i0 + lane;
@@ -401,11 +300,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                         const int j1 = cur.cptr[c + 1];
                         for (int j = cur.cptr[c]; j < j1; ++j) {
                             const int2 run = cur.rptr[j];
-#ifdef FV_CHAIN_EXP_SAMEADDR
-                            bulk_g2s_hint(dst + (size_t)(run.y >> 16) * ROW_BYTES, src_l + (size_t)(run.x & 15) * ROW_BYTES,
-#else
                             bulk_g2s_hint(dst + (size_t)(run.y >> 16) * ROW_BYTES, src + (size_t)run.x * ROW_BYTES,
-#endif
                                           (uint32_t)(run.y & 0xffff) * ROW_BYTES, bar_full + slot, kv_pol);
                         }
                     }
@@ -462,12 +357,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
     int ju = 0;                                               // slots done
     if (last) for (int i = tid; i < MB_MAX * RMAX; i += NWC * 32) sh_logq[i] = 0.0;
 
-#ifdef FV_CHAIN_PROF
-    long long pf[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, pt = clock64(), rp[4] = {0, 0, 0, 0};
-#define PF(i) do { const long long now_ = clock64(); pf[i] += now_ - pt; pt = now_; } while (0)
-#else
-#define PF(i) do { } while (0)
-#endif
     for (int t = 0; t < N; ++t) {
         const int me0 = __ldg(m.mask_rowptr + t);
         const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
@@ -492,12 +381,10 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             float* sh_u = sh_ubuf + buf * RMAX;
             if (last && tid < RMAX) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
-            PF(0);
             // ---- LN1 (Alg. 2 l.12) -> B tile ----------------------------------------------------------------------
             for (int r = warp; r < n_own; r += NWC) ln_row_btile(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_bact, r, lane);
             umma::fence_smem_to_async();
             cbar();
-            PF(1);
             // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13): D[feature, sample] = W_qkv[tile] . a^T -------------------------
             // (four issuing threads, one per M-tile: a small tcgen05.mma costs its issuing thread ~45 cycles, the
             // tensor pipe ~10, so the tiles are issued concurrently from four warps)
@@ -515,7 +402,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             mbar_wait(bar_mma, mma_par); mma_par ^= 1u;
             umma::fence_after_sync();
-            PF(2);
             if (warp < 12) {
                 const int mt = warp >> 2, fl = (warp & 3) * 32 + lane;
                 float v[NC];
@@ -531,7 +417,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             umma::fence_before_sync();
             cbar();
-            PF(3);
             // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) ---------------------------------
             for (int i = tid; i < RMAX * (2 * D / 8); i += NWC * 32) {
                 const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
@@ -540,8 +425,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                 __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
                 *reinterpret_cast<uint4*>(dst) = v;
             }
-            if (FV_CHAIN_RING) asm volatile("fence.proxy.async.global;\n" ::: "memory");   // the producer reads these rows by cp.async.bulk
-            PF(11);
+            asm volatile("fence.proxy.async.global;\n" ::: "memory");   // the producer reads these rows by cp.async.bulk
             // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---------------------------
             for (int task = warp; task < RMAX * NSPLIT; task += NWC) {
                 const int r = task / NSPLIT, sp = task - r * NSPLIT;
@@ -567,33 +451,13 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                         for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + sub * 8 + j]);
                     }
                 }
-                if (!FV_CHAIN_RING) {
-                    attend_gather<NSPLIT>(q, reinterpret_cast<const unsigned char*>(m.kv + ((size_t)(b_first + r) * NL + l) * N * (2 * D)),
-                                          m.mask_col + me0, nn, sp, rg, sub, mm, ll, acc);
-                } else {
-                    for (int c = sp; c < nch; c += NSPLIT) {
-                        const int kr = r / GR, nk = min(GR, n_own - kr * GR);
-                        const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
-                        uint32_t slot;
-#ifdef FV_CHAIN_PROF
-                        const long long r0 = clock64();
-                        slot = sq % NSLOT;
-                        while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
-                        const long long r1 = clock64();
-                        mbar_wait(rc.bar_full + slot, (sq / NSLOT) & 1u);
-                        const long long r2 = clock64();
-                        const unsigned char* chunk = rc.ring + (size_t)slot * CHUNK_BYTES;
-                        attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
-                        const long long r3 = clock64();
-                        ring_release(rc, slot, lane);
-                        const long long r4 = clock64();
-                        rp[0] += r1 - r0; rp[1] += r2 - r1; rp[2] += r3 - r2; rp[3] += r4 - r3;
-#else
-                        const unsigned char* chunk = ring_acquire<NSLOT, CHUNK_BYTES>(rc, sq, slot);
-                        attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
-                        ring_release(rc, slot, lane);
-#endif
-                    }
+                for (int c = sp; c < nch; c += NSPLIT) {
+                    const int kr = r / GR, nk = min(GR, n_own - kr * GR);
+                    const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
+                    uint32_t slot;
+                    const unsigned char* chunk = ring_acquire<NSLOT, CHUNK_BYTES>(rc, sq, slot);
+                    attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
+                    ring_release(rc, slot, lane);
                 }
 #pragma unroll
                 for (int o = LPR; o < 32; o <<= 1) {       // merge the row groups of the warp
@@ -624,7 +488,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             seq_base += (uint32_t)(n_own * nch);
             cbar();
-            PF(4);
             if (tid == 0) st_release_s32(sh_app, ju + 1);
             if (NSPLIT > 1) {                       // combine the split partials, fixed order
                 for (int i = tid; i < RMAX * D; i += NWC * 32) {
@@ -645,12 +508,10 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                 }
                 cbar();
             }
-            PF(5);
             // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) -> B tile ------------------------------------------
             for (int r = warp; r < n_own; r += NWC) ln_row_btile(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_bact, r, lane);
             umma::fence_smem_to_async();
             cbar();
-            PF(6);
             // ---- FFN up-projection + exact GELU -> hidden B tile [16 x 512] ---------------------------------------
             if (warp < 4 && lane == 0) {
                 umma::fence_after_sync();
@@ -662,7 +523,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             mbar_wait(bar_mma, mma_par); mma_par ^= 1u;
             umma::fence_after_sync();
-            PF(7);
             {
                 const int mt = warp >> 2, jl = (warp & 3) * 32 + lane, j = mt * 128 + jl;     // hidden unit
                 float v[NC];
@@ -677,7 +537,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             umma::fence_smem_to_async();
             umma::fence_before_sync();
             cbar();
-            PF(8);
             // ---- FFN down-projection (A = W_2 image in shared memory) + residual (Alg. 2 l.16) --------------------------
             // (K = 512 split over the four issuers: four partial accumulators, summed in the epilogue in fixed order)
             if (warp < 4 && lane == 0) {
@@ -692,7 +551,6 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             }
             mbar_wait(bar_mma, mma_par); mma_par ^= 1u;
             umma::fence_after_sync();
-            PF(9);
             if (warp < 4) {
                 const int f = warp * 32 + lane;
                 float v[NC];
@@ -749,15 +607,8 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             } else {
                 umma::fence_before_sync();
             }
-            PF(10);
         }
     }
-#ifdef FV_CHAIN_PROF
-    if (tid == 0 && chain == 0)
-        printf("layer %d cycles/slot: in %lld ln1 %lld qkv %lld epi %lld att %lld comb %lld ln2 %lld ffn1 %lld gelu %lld ffn2 %lld out %lld append %lld (slots %d)\n",
-               l, pf[0] / ju, pf[1] / ju, pf[2] / ju, pf[3] / ju, pf[4] / ju, pf[5] / ju, pf[6] / ju, pf[7] / ju, pf[8] / ju, pf[9] / ju, pf[10] / ju, pf[11] / ju, ju);
-    if (tid == 0 && chain == 0) printf("layer %d ring cycles/slot: wait-issued %lld wait-full %lld compute %lld release %lld\n", l, rp[0] / ju, rp[1] / ju, rp[2] / ju, rp[3] / ju);
-#endif
     cbar();
     umma::fence_before_sync();
     cluster_sync_all();                                       // no CTA leaves while a peer may still write to it

@@ -244,6 +244,49 @@ def test_cluster_decode_variant(monkeypatch):
     print(f"cluster decode: near-tie sites {ties}, flips among them {flips}")
 
 
+CHAIN_CASES = {
+    "sk_causal_4l": ("cfg3", dict(L=100, n_sites=100), 41),
+    "ea3d_4l": ("cfg4", dict(L=5, n_sites=125, window=16), 150),
+    "ea2d_6l": ("cfg5", dict(L=12, n_sites=144, window=12), 19),
+    "ea2d_6l_B300": ("cfg5", dict(L=16, n_sites=256, window=16, n_layers=6), 300),
+    "ea2d_2l_16_per_microbatch": ("cfg5", dict(L=6, n_sites=36, window=6, n_layers=2), 2300),
+    "ea2d_1l": ("cfg5", dict(L=6, n_sites=36, window=6, n_layers=1), 77),
+    "ln2_style_1": ("cfg5", dict(L=6, n_sites=36, window=6, n_layers=3, ln2_style=1), 45),
+}
+
+
+@pytest.mark.parametrize("case", list(CHAIN_CASES))
+def test_chain_sampler(case, monkeypatch):
+    """FLASHVAN_DECODE=chain: the weight-stationary sampler (fv_chain.cu: clusters of n_layers CTAs, tcgen05 GEMMs
+    with the weights in tensor / shared memory, DSMEM hand-off) against the oracle, exactly like the default
+    kernel: 1 to 8 layers' worth of cluster sizes, micro-batches of 1..16 samples, ragged last micro-batch."""
+    base, kw, B = CHAIN_CASES[case]
+    w = dataclasses.replace(W.CONFIGS[base], **kw)
+    model, weights, posemb, rp, col = build(w, B)
+    monkeypatch.setenv("FLASHVAN_DECODE", "chain")
+    assert model.sampler_kind(B) == "chain"
+    ties, flips = check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B))
+    print(f"chain sampler {case}: near-tie sites {ties}, flips among them {flips}")
+    u = dev(W.make_uniforms(w, B, seed=11))
+    a = model.sample(u, want_cond_p=True)
+    b = model.sample(u, want_cond_p=True)
+    assert all(torch.equal(x, y) for x, y in zip(a, b))              # bit-reproducible
+    for Bs in (1, 7, 9):                                              # ragged: fewer chains / micro-batches than the pool
+        if Bs <= B:
+            check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, Bs, seed=Bs))
+    model.close()
+
+
+def test_chain_sampler_refuses_uncovered_shapes(monkeypatch):
+    w = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2)       # d = 64
+    model, weights, posemb, rp, col = build(w, 8)
+    monkeypatch.setenv("FLASHVAN_DECODE", "chain")
+    assert model.sampler_kind(8) == "ring"
+    with pytest.raises(fv.FlashVanError, match="chain"):
+        model.sample(dev(W.make_uniforms(w, 8)))
+    model.close()
+
+
 def test_sample_is_reproducible_across_fresh_models():
     """Bit-reproducibility (include/flashvan.h) must not depend on what the KV pool or shared memory
     held before: the same uniforms through several freshly created models, cold caches included.
