@@ -93,23 +93,39 @@ __device__ __forceinline__ void ln8_to_tile(float4 (&x)[D / 32], const float* __
     }
 }
 
-// Exact-GELU 0.5 x (1 + erf(x / sqrt 2)) with erf from Abramowitz-Stegun 7.1.26 (|error| <= 1.5e-7,
-// far below the bf16 rounding of the result): erf(z) = 1 - (a1 t + .. + a5 t^5) exp(-z^2),
-// t = 1 / (1 + p z), z = |x| / sqrt 2.  Written in y = |x| sqrt(log2(e) / 2), so that
-// exp(-z^2) = 2^(-y y) needs no further scaling: one rcp.approx, one ex2.approx and ten FP32
-// instructions -- the epilogue of the fused FFN evaluates 4d of these per row and bounds the kernel.
-__device__ __forceinline__ float gelu_fast(float x) {
-    const float hx = 0.5f * x;
-    const float y = fabsf(x) * 0.84932180028801904f;           // sqrt(log2(e) / 2)
-    float t, ex;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(fmaf(0.27273748f, y, 1.0f)));   // p / sqrt(2) / 0.849..
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(-y * y));
-    float p = fmaf(1.061405429f, t, -1.453152027f);
-    p = fmaf(p, t, 1.421413741f);
-    p = fmaf(p, t, -0.284496736f);
-    p = fmaf(p, t, 0.254829592f);
-    const float e = fmaf(-p * t, ex, 1.0f);                    // erf(|x| / sqrt 2)
-    return fmaf(fabsf(hx), e, hx);                             // 0.5 x (1 + sign(x) e)
+// erfc-based exact-GELU with ONE special-function instruction: Phi(-|x|) = 0.5 erfc(|x| / sqrt 2) = 2^P(|x|) with a
+// degree-6 polynomial P fitted on [0, 10] (max |error| of the GELU 5e-8 in exact arithmetic, 5e-7 in fp32 --
+// below the bf16 rounding of the result by four orders of magnitude); gelu(x) = max(x, 0) - |x| Phi(-|x|).
+// P(a) = -0.9999930605 - 1.151201707 a - 0.4587709584 a^2 - 0.05341212449 a^3 + 8.080729771e-3 a^4
+//        - 7.692237508e-4 a^5 + 3.309327859e-5 a^6, |x| clamped to 10 (beyond it Phi(-|x|) < 1e-23).
+// Two of them at once on the packed fp32 pipe (fma.rn.f32x2: one instruction, two FMAs) -> one bf16x2 word.
+__device__ __forceinline__ uint64_t f2pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t gelu_erfc_x2(float x0, float x1) {
+    const float a0 = fminf(fabsf(x0), 10.0f), a1 = fminf(fabsf(x1), 10.0f);
+    const uint64_t ax = f2pack(a0, a1);
+    uint64_t p = ffma2(f2pack(3.309327859e-05f, 3.309327859e-05f), ax, f2pack(-7.692237508e-04f, -7.692237508e-04f));
+    p = ffma2(p, ax, f2pack(8.080729771e-03f, 8.080729771e-03f));
+    p = ffma2(p, ax, f2pack(-5.341212449e-02f, -5.341212449e-02f));
+    p = ffma2(p, ax, f2pack(-4.587709584e-01f, -4.587709584e-01f));
+    p = ffma2(p, ax, f2pack(-1.151201707e+00f, -1.151201707e+00f));
+    p = ffma2(p, ax, f2pack(-9.999930605e-01f, -9.999930605e-01f));
+    float p0, p1, e0, e1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(p));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(p0));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(p1));
+    const uint64_t g = ffma2(f2pack(-a0, -a1), f2pack(e0, e1), f2pack(fmaxf(x0, 0.f), fmaxf(x1, 0.f)));
+    float g0, g1;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(g0), "=f"(g1) : "l"(g));
+    return pack_bf16(g0, g1);
 }
 
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
@@ -636,17 +652,21 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
     auto issue_w2 = [&](long long c) {                       // thread 0: W2 of chunk c -> slot c & 1
         bulk_in(sW2 + (int)(c & 1) * G::W2_BYTES, a.w_img + (size_t)(c % G::NHC) * G::WBUF + G::W1_BYTES, G::W2_BYTES, &bar_w2[c & 1]);
     };
+    const uint64_t dA = umma::make_desc_sw128(umma::smem_u32(sA)), dH = umma::make_desc_sw128(umma::smem_u32(sH));
+    const uint64_t dW1 = umma::make_desc_sw128(umma::smem_u32(sW1)), dW2 = umma::make_desc_sw128(umma::smem_u32(sW2));
     auto issue_mma1 = [&](long long c) {                     // thread 0: acc1[c & 1] = A W1_c^T
         umma::mbar_wait(&bar_w1[c & 1], (uint32_t)((c >> 1) & 1));
         umma::fence_after_sync();
-        const uint32_t a0 = umma::smem_u32(sA), b0 = umma::smem_u32(sW1 + (int)(c & 1) * G::W1_BYTES);
+        // descriptors = one base per operand + compile-time offsets: the issuing thread pays ~45 cycles per tcgen05.mma
+        // as it is, and every instruction spent on rebuilding descriptors delays the whole epilogue of its warp
+        const uint64_t b0 = dW1 + (uint64_t)(((int)(c & 1) * G::W1_BYTES) >> 4);
         const uint32_t acc = tmem + (uint32_t)(c & 1) * G::HC;
 #pragma unroll
         for (int kb = 0; kb < G::KB; ++kb)
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks)
-                umma::mma_bf16_ss(acc, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
-                                  umma::make_desc_sw128(b0 + kb * (G::HC * 128) + ks * 32), idesc1, (kb | ks) != 0);
+                umma::mma_bf16_ss(acc, dA + (uint64_t)((kb * (TM * 128) + ks * 32) >> 4),
+                                  b0 + (uint64_t)((kb * (G::HC * 128) + ks * 32) >> 4), idesc1, (kb | ks) != 0);
         umma::commit(&bar_m1[c & 1]);
     };
     if (tid == 0 && n_chunks > 0) {
@@ -723,10 +743,10 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
                     for (int c = 0; c < 2; ++c) {
                         const float4 ba = bq[2 * c], bb = bq[2 * c + 1];
                         uint32_t p[4];
-                        p[0] = pack_bf16(gelu_fast(v[c * 8 + 0] + ba.x), gelu_fast(v[c * 8 + 1] + ba.y));
-                        p[1] = pack_bf16(gelu_fast(v[c * 8 + 2] + ba.z), gelu_fast(v[c * 8 + 3] + ba.w));
-                        p[2] = pack_bf16(gelu_fast(v[c * 8 + 4] + bb.x), gelu_fast(v[c * 8 + 5] + bb.y));
-                        p[3] = pack_bf16(gelu_fast(v[c * 8 + 6] + bb.z), gelu_fast(v[c * 8 + 7] + bb.w));
+                        p[0] = gelu_erfc_x2(v[c * 8 + 0] + ba.x, v[c * 8 + 1] + ba.y);
+                        p[1] = gelu_erfc_x2(v[c * 8 + 2] + ba.z, v[c * 8 + 3] + ba.w);
+                        p[2] = gelu_erfc_x2(v[c * 8 + 4] + bb.x, v[c * 8 + 5] + bb.y);
+                        p[3] = gelu_erfc_x2(v[c * 8 + 6] + bb.z, v[c * 8 + 7] + bb.w);
                         // H is GEMM 2's operand: the previous chunk's GEMM 2 (issued one pass ago,
                         // behind it only this chunk's GEMM 1) must have read it before the first store
                         if (hf == 0 && c == 0 && j > 0) {
@@ -749,13 +769,13 @@ __global__ void __launch_bounds__(FFN_THREADS, 2) lp_ffn_kernel(const __grid_con
             if (tid == 0) {                            // GEMM 2 of this chunk
                 umma::fence_after_sync();
                 umma::mbar_wait(&bar_w2[g & 1], (uint32_t)((g >> 1) & 1));
-                const uint32_t h0 = umma::smem_u32(sH), b0 = umma::smem_u32(sW2 + (int)(g & 1) * G::W2_BYTES);
+                const uint64_t b0 = dW2 + (uint64_t)(((int)(g & 1) * G::W2_BYTES) >> 4);
 #pragma unroll
                 for (int kb = 0; kb < G::HC / 64; ++kb)
 #pragma unroll
                     for (int ks = 0; ks < 4; ++ks)
-                        umma::mma_bf16_ss(tmem_acc2, umma::make_desc_sw128(h0 + kb * (TM * 128) + ks * 32),
-                                          umma::make_desc_sw128(b0 + kb * (D * 128) + ks * 32), idesc2, (j | kb | ks) != 0);
+                        umma::mma_bf16_ss(tmem_acc2, dH + (uint64_t)((kb * (TM * 128) + ks * 32) >> 4),
+                                          b0 + (uint64_t)((kb * (D * 128) + ks * 32) >> 4), idesc2, (j | kb | ks) != 0);
                 umma::commit(&bar_m2);
             }
         }
