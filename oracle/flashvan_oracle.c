@@ -19,8 +19,11 @@
  * emits the conditional of spin t (Alg. 2).
  *
  * Weights blob (fp32, promoted to fp64 here), row-major [out,in], y = W x + b (Eq. 2, l.98):
- *   tok_emb[2,d_token]; per layer: ln1_g[d] ln1_b[d] Wq[d,d] bq[d] Wk[d,d] bk[d] Wv[d,d] bv[d]
- *   (Wo[d,d] bo[d] iff has_wo) ln2_g[d] ln2_b[d] W1[f,d] b1[f] W2[d,f] b2[d]; head_W[2,d] head_b[2].
+ *   tok_emb[V,d_token]; per layer: ln1_g[d] ln1_b[d] Wq[d,d] bq[d] Wk[d,d] bk[d] Wv[d,d] bv[d]
+ *   (Wo[d,d] bo[d] iff has_wo) ln2_g[d] ln2_b[d] W1[f,d] b1[f] W2[d,f] b2[d]; head_W[V,d] head_b[V].
+ * V = 2 (one spin per token) everywhere except in the patch-token functions at the end of the file, where a
+ * token stands for a patch of 2^D spins and V = 2^(2^D) (SI I.D; the parameter counts
+ * "w/ patch" of Table 7, l.765-771, fix that the embedding has V rows and the head V logits and biases).
  */
 #include <math.h>
 #include <stdint.h>
@@ -30,6 +33,7 @@
 typedef struct {
     int32_t n_sites, n_layers, d_model, n_heads, d_token, ffn_mult, has_wo, act, ln2_style;
     double ln_eps;
+    int32_t vocab;      /* tokens: 2 for one spin per token; 2^(2^D) with 2^D-spin patches (l.603-605) */
 } fvo_config;
 
 typedef struct {
@@ -46,14 +50,14 @@ typedef struct {
 static int64_t blob_size(const fvo_config *c) {
     int64_t d = c->d_model, f = (int64_t)c->ffn_mult * d;
     int64_t per = 2 * d + 3 * (d * d + d) + (c->has_wo ? d * d + d : 0) + 2 * d + f * d + f + d * f + d;
-    return 2 * (int64_t)c->d_token + c->n_layers * per + 2 * d + 2;
+    return c->vocab * (int64_t)c->d_token + c->n_layers * per + c->vocab * d + c->vocab;
 }
 
 int64_t fvo_n_weights(const fvo_config *c) { return blob_size(c); }
 
 static void carve(const fvo_config *c, const float *w, model_w *m) {
     int64_t d = c->d_model, f = (int64_t)c->ffn_mult * d;
-    m->tok_emb = w; w += 2 * c->d_token;
+    m->tok_emb = w; w += c->vocab * c->d_token;
     for (int l = 0; l < c->n_layers; ++l) {
         layer_w *L = &m->layer[l];
         L->ln1_g = w; w += d; L->ln1_b = w; w += d;
@@ -65,7 +69,7 @@ static void carve(const fvo_config *c, const float *w, model_w *m) {
         L->w1 = w; w += f * d; L->b1 = w; w += f;
         L->w2 = w; w += d * f; L->b2 = w; w += d;
     }
-    m->head_w = w; w += 2 * d; m->head_b = w;
+    m->head_w = w; w += c->vocab * d; m->head_b = w;
 }
 
 /* LayerNorm over the feature axis: mean, BIASED variance, eps inside the sqrt, affine.
@@ -297,4 +301,123 @@ void fvo_energy_csr(int32_t B, int32_t N, const int8_t *spins, const int32_t *ro
             for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) e -= (double)val[k] * s[i] * s[col[k]];
         E[b] = e;
     }
+}
+
+/* =======================================================================================
+ * Patch tokens (SI I.D): "the input spin configuration on an L^D lattice is
+ * partitioned into non-overlapping patches of size 2^D.  Each patch is mapped to a token, reducing
+ * the input sequence length from L^D to (L/2)^D."  The model is unchanged except for its two ends:
+ * the embedding table has V = 2^(2^D) rows and the head emits V logits (parameter counts of Table 7,
+ * l.765-771).  A token is drawn from Categorical(softmax(z)) (Alg. 2 l.358-359); with a caller-supplied
+ * uniform that is the inverse-CDF rule in token order: the first k with u < p_0 + ... + p_k (reading
+ * A10 carried over; the last token if rounding leaves u above the total).  Which bit of a token is
+ * which spin of the patch is an index list of the workload (workloads.py), not part of this file.
+ * probs [B,N,V] (may be NULL) receives the full conditional distribution of every position.
+ * ===================================================================================== */
+static void head_probs(const fvo_config *c, const model_w *m, const double *h, double *z) {
+    int V = c->vocab;
+    linear(V, c->d_model, m->head_w, m->head_b, h, z);
+    double mx = z[0];
+    for (int k = 1; k < V; ++k) if (z[k] > mx) mx = z[k];
+    double den = 0.0;
+    for (int k = 0; k < V; ++k) { z[k] = exp(z[k] - mx); den += z[k]; }
+    for (int k = 0; k < V; ++k) z[k] /= den;
+}
+
+int fvo_tok_sample(const fvo_config *c, const float *weights, const float *posemb,
+                   const int32_t *rowptr, const int32_t *col, int32_t B, const float *uniforms,
+                   int32_t *tokens, double *logq, double *probs) {
+    int N = c->n_sites, d = c->d_model, f = c->ffn_mult * d, nl = c->n_layers, V = c->vocab;
+    int err = 0;
+#pragma omp parallel
+    {
+        layer_w *lw = (layer_w *)malloc(sizeof(layer_w) * nl);
+        model_w m; m.layer = lw; carve(c, weights, &m);
+        double *K = (double *)malloc(sizeof(double) * (size_t)nl * N * d);
+        double *Vv = (double *)malloc(sizeof(double) * (size_t)nl * N * d);
+        double *h = (double *)malloc(sizeof(double) * (5 * d + 2 * f + N + V));
+        double *a = h + d, *q = a + d, *u = q + d, *tmp = u + d, *score = tmp + 2 * d + f, *p = score + N;
+        if (!K || !Vv || !h) {
+#pragma omp atomic write
+            err = -1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int b = 0; b < B; ++b) {
+                double lq = 0.0;
+                int prev_tok = 0;                                   /* start token, l.323 */
+                for (int t = 0; t < N; ++t) {
+                    embed(c, &m, posemb, prev_tok, t, h);
+                    for (int l = 0; l < nl; ++l) {
+                        const layer_w *L = &lw[l];
+                        double *Kl = K + (size_t)l * N * d, *Vl = Vv + (size_t)l * N * d;
+                        layer_norm(d, h, L->ln1_g, L->ln1_b, c->ln_eps, a);
+                        linear(d, d, L->wq, L->bq, a, q);
+                        linear(d, d, L->wk, L->bk, a, Kl + (size_t)t * d);
+                        linear(d, d, L->wv, L->bv, a, Vl + (size_t)t * d);
+                        attend(c, q, Kl, Vl, col + rowptr[t], rowptr[t + 1] - rowptr[t], u, score);
+                        post_attention(c, L, h, u, tmp);
+                    }
+                    head_probs(c, &m, h, p);                                   /* l.358 */
+                    double uu = (double)uniforms[(size_t)b * N + t], cdf = 0.0;
+                    int tok = V - 1;
+                    for (int k = 0; k < V; ++k) { cdf += p[k]; if (uu < cdf) { tok = k; break; } }   /* l.359 */
+                    tokens[(size_t)b * N + t] = tok;
+                    lq += log(p[tok]);
+                    if (probs) for (int k = 0; k < V; ++k) probs[((size_t)b * N + t) * V + k] = p[k];
+                    prev_tok = tok;
+                }
+                logq[b] = lq;
+            }
+        }
+        free(K); free(Vv); free(h); free(lw);
+    }
+    return err;
+}
+
+int fvo_tok_log_prob(const fvo_config *c, const float *weights, const float *posemb,
+                     const int32_t *rowptr, const int32_t *col, int32_t B, const int32_t *tokens,
+                     double *logq, double *probs) {
+    int N = c->n_sites, d = c->d_model, f = c->ffn_mult * d, nl = c->n_layers, V = c->vocab;
+    int err = 0;
+#pragma omp parallel
+    {
+        layer_w *lw = (layer_w *)malloc(sizeof(layer_w) * nl);
+        model_w m; m.layer = lw; carve(c, weights, &m);
+        double *X = (double *)malloc(sizeof(double) * (size_t)N * d * 4);
+        double *Q = X + (size_t)N * d, *K = Q + (size_t)N * d, *Vv = K + (size_t)N * d;
+        double *a = (double *)malloc(sizeof(double) * (4 * d + 2 * f + N + V));
+        double *u = a + d, *tmp = u + d, *score = tmp + 2 * d + f, *p = score + N;
+        if (!X || !a) {
+#pragma omp atomic write
+            err = -1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int b = 0; b < B; ++b) {
+                const int32_t *s = tokens + (size_t)b * N;
+                for (int t = 0; t < N; ++t) embed(c, &m, posemb, t == 0 ? 0 : s[t - 1], t, X + (size_t)t * d);
+                for (int l = 0; l < nl; ++l) {
+                    const layer_w *L = &lw[l];
+                    for (int t = 0; t < N; ++t) {
+                        layer_norm(d, X + (size_t)t * d, L->ln1_g, L->ln1_b, c->ln_eps, a);
+                        linear(d, d, L->wq, L->bq, a, Q + (size_t)t * d);
+                        linear(d, d, L->wk, L->bk, a, K + (size_t)t * d);
+                        linear(d, d, L->wv, L->bv, a, Vv + (size_t)t * d);
+                    }
+                    for (int t = 0; t < N; ++t) {
+                        attend(c, Q + (size_t)t * d, K, Vv, col + rowptr[t], rowptr[t + 1] - rowptr[t], u, score);
+                        post_attention(c, L, X + (size_t)t * d, u, tmp);
+                    }
+                }
+                double lq = 0.0;
+                for (int t = 0; t < N; ++t) {
+                    head_probs(c, &m, X + (size_t)t * d, p);
+                    lq += log(p[s[t]]);
+                    if (probs) for (int k = 0; k < V; ++k) probs[((size_t)b * N + t) * V + k] = p[k];
+                }
+                logq[b] = lq;
+            }
+        }
+        free(X); free(a); free(lw);
+    }
+    return err;
 }

@@ -23,7 +23,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 class _Cfg(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
                 ("n_sites", "n_layers", "d_model", "n_heads", "d_token", "ffn_mult",
-                 "has_wo", "act", "ln2_style")] + [("ln_eps", ctypes.c_double)]
+                 "has_wo", "act", "ln2_style")] + [("ln_eps", ctypes.c_double), ("vocab", ctypes.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -45,6 +45,8 @@ def _load():
         _lib.fvo_n_weights.restype = ctypes.c_int64
         _lib.fvo_sample.restype = ctypes.c_int
         _lib.fvo_log_prob.restype = ctypes.c_int
+        _lib.fvo_tok_sample.restype = ctypes.c_int
+        _lib.fvo_tok_log_prob.restype = ctypes.c_int
         _lib.fvo_energy_dense.restype = None
         _lib.fvo_energy_csr.restype = None
     return _lib
@@ -52,7 +54,7 @@ def _load():
 
 def _cfg(w) -> _Cfg:
     return _Cfg(w.n_sites, w.n_layers, w.d_model, w.n_heads, w.d_token, w.ffn_mult,
-                w.has_wo, 0, w.ln2_style, float(w.ln_eps))
+                w.has_wo, 0, w.ln2_style, float(w.ln_eps), int(getattr(w, "vocab", 2)))
 
 
 def _p(a):
@@ -106,6 +108,55 @@ def log_prob(w, weights, posemb, rowptr, col, spins):
     if rc != 0:
         raise MemoryError("oracle log_prob failed")
     return logq, cp
+
+
+def tok_sample(w, weights, posemb, rowptr, col, uniforms):
+    """Alg. 2 with patch tokens: inverse-CDF draw of one of w.vocab tokens per position.
+    Returns tokens int32 [B,N], logq f64 [B], probs f64 [B,N,V] (the full conditional of every position)."""
+    lib = _load()
+    weights, posemb = _c(weights, np.float32), _c(posemb, np.float32)
+    rowptr, col = _c(rowptr, np.int32), _c(col, np.int32)
+    uniforms = _c(uniforms, np.float32)
+    assert weights.size == n_weights(w) and posemb.shape == (w.n_sites, w.d_pos)
+    B = uniforms.shape[0]
+    tokens = np.empty((B, w.n_sites), np.int32)
+    logq = np.empty(B, np.float64)
+    probs = np.empty((B, w.n_sites, w.vocab), np.float64)
+    rc = lib.fvo_tok_sample(ctypes.byref(_cfg(w)), _p(weights), _p(posemb), _p(rowptr), _p(col),
+                            ctypes.c_int32(B), _p(uniforms), _p(tokens), _p(logq), _p(probs))
+    if rc != 0:
+        raise MemoryError("oracle tok_sample failed")
+    return tokens, logq, probs
+
+
+def tok_log_prob(w, weights, posemb, rowptr, col, tokens):
+    """Alg. 1 with patch tokens: log q of given token sequences and the full conditionals [B,N,V]."""
+    lib = _load()
+    weights, posemb = _c(weights, np.float32), _c(posemb, np.float32)
+    rowptr, col = _c(rowptr, np.int32), _c(col, np.int32)
+    tokens = _c(tokens, np.int32)
+    assert weights.size == n_weights(w) and posemb.shape == (w.n_sites, w.d_pos)
+    assert tokens.min() >= 0 and tokens.max() < w.vocab
+    B = tokens.shape[0]
+    logq = np.empty(B, np.float64)
+    probs = np.empty((B, w.n_sites, w.vocab), np.float64)
+    rc = lib.fvo_tok_log_prob(ctypes.byref(_cfg(w)), _p(weights), _p(posemb), _p(rowptr), _p(col),
+                              ctypes.c_int32(B), _p(tokens), _p(logq), _p(probs))
+    if rc != 0:
+        raise MemoryError("oracle tok_log_prob failed")
+    return logq, probs
+
+
+def tokens_to_spins(tokens, site_index):
+    """Unpack patch tokens into lattice spins: bit k of token n is the spin of lattice site site_index[n, k]
+    (the index list comes from workloads.patch_site_index), spin = 2 bit - 1."""
+    tokens = np.asarray(tokens, np.int64)
+    B, n_tok = tokens.shape
+    P = site_index.shape[1]
+    spins = np.zeros((B, n_tok * P), np.int8)
+    for k in range(P):
+        spins[:, site_index[:, k]] = (2 * ((tokens >> k) & 1) - 1).astype(np.int8)
+    return spins
 
 
 def energy_dense(spins, J):

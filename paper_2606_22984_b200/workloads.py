@@ -43,10 +43,16 @@ class Workload:
     has_wo: int = 0
     ln2_style: int = 0
     ln_eps: float = 1e-5
+    vocab: int = 2        # tokens; 2^(patch^dim) when a token stands for a patch of spins
+    patch: int = 1        # linear patch size: the model's lattice (L, n_sites) is then the lattice of PATCHES
 
     @property
     def d_pos(self) -> int:
         return self.d_model - self.d_token
+
+    @property
+    def spins_per_token(self) -> int:
+        return self.patch ** self.dim if self.patch > 1 else 1
 
 
 CONFIGS = {
@@ -71,7 +77,7 @@ def weight_segments(w: Workload):
 
     Matrices are row-major [out, in] (y = W x + b, Eq. 2)."""
     d, f = w.d_model, w.ffn_mult * w.d_model
-    segs = [("tok_emb", (2, w.d_token))]
+    segs = [("tok_emb", (w.vocab, w.d_token))]
     for l in range(w.n_layers):
         p = f"l{l}."
         segs += [(p + "ln1_g", (d,)), (p + "ln1_b", (d,)),
@@ -83,7 +89,7 @@ def weight_segments(w: Workload):
         segs += [(p + "ln2_g", (d,)), (p + "ln2_b", (d,)),
                  (p + "w1", (f, d)), (p + "b1", (f,)),
                  (p + "w2", (d, f)), (p + "b2", (d,))]
-    segs += [("head_w", (2, d)), ("head_b", (2,))]
+    segs += [("head_w", (w.vocab, d)), ("head_b", (w.vocab,))]
     return segs
 
 
@@ -132,6 +138,45 @@ def make_spins(w: Workload, batch: int, seed: int = 11) -> np.ndarray:
     """Uniform random +-1 configurations (teacher-forced inputs for tests)."""
     rng = np.random.default_rng(seed)
     return (2 * rng.integers(0, 2, size=(batch, w.n_sites)) - 1).astype(np.int8)
+
+
+def make_tokens(w: Workload, batch: int, seed: int = 11) -> np.ndarray:
+    """Uniform random token ids in [0, vocab) (teacher-forced inputs of a patched model)."""
+    rng = np.random.default_rng(seed)
+    return rng.integers(0, w.vocab, size=(batch, w.n_sites)).astype(np.int32)
+
+
+# ------------------------------------------------------------------------------ patches
+def patched(w: Workload, patch: int = 2) -> Workload:
+    """The patched model of an EA workload: one token per patch^dim block of spins, so the
+    model's lattice is the lattice of patches (L / patch per side) and the vocabulary has 2^(patch^dim) tokens."""
+    assert w.model == "ea" and w.patch == 1 and w.L % patch == 0
+    Lt = w.L // patch
+    return dataclasses.replace(w, L=Lt, n_sites=Lt ** w.dim, patch=patch, vocab=2 ** (patch ** w.dim))
+
+
+def spin_lattice(w: Workload) -> Workload:
+    """The lattice of SPINS under a patched model (couplings and energies live there)."""
+    if w.patch == 1:
+        return w
+    Ls = w.L * w.patch
+    return dataclasses.replace(w, L=Ls, n_sites=Ls ** w.dim, patch=1, vocab=2)
+
+
+def patch_site_index(w: Workload) -> np.ndarray:
+    """[n_tokens, patch^dim] int32: the lattice site (raster index on the spin lattice) whose spin is bit k of
+    token n.  Tokens in raster order of the patch lattice; inside a patch the offsets in raster order as well
+    (last coordinate fastest), bit 0 = the patch's first site."""
+    assert w.patch > 1
+    D, p, Lt, Ls = w.dim, w.patch, w.L, w.L * w.patch
+    out = np.zeros((w.n_sites, p ** D), dtype=np.int32)
+    for n, tc in enumerate(itertools.product(range(Lt), repeat=D)):
+        for k, oc in enumerate(itertools.product(range(p), repeat=D)):
+            site = 0
+            for a in range(D):
+                site = site * Ls + tc[a] * p + oc[a]
+            out[n, k] = site
+    return out
 
 
 # --------------------------------------------------------------------------- couplings
@@ -257,5 +302,7 @@ def make_all(w: Workload, batch: Optional[int] = None, u_seed: int = SEED_U) -> 
     if w.model == "sk":
         out["J"] = make_couplings_sk(w)
     else:
-        out["bond_rowptr"], out["bond_col"], out["bond_val"] = make_couplings_ea(w)
+        out["bond_rowptr"], out["bond_col"], out["bond_val"] = make_couplings_ea(spin_lattice(w))
+        if w.patch > 1:
+            out["site_index"] = patch_site_index(w)
     return out
