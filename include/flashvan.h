@@ -52,14 +52,18 @@ typedef struct {
     int32_t ln2_style; /* 0: h += FFN(LN2(h)) (Alg. 2 l.346); 1: h = LN2(h); h += FFN(h)      */
                        /*    (Alg. 1 l.237-239); reading A1                                   */
     int32_t max_batch; /* KV pool is sized for this many samples                              */
+    int32_t vocab;     /* tokens: 2 = one spin per token (0 is read as 2); 16 or 256 = one token  */
+                       /*    per patch of 4 / 8 spins (SI I.D, l.603-605; needs d_model <= 128,    */
+                       /*    has_wo = 0): embedding and head then have `vocab` rows, tokens are    */
+                       /*    drawn by inverse CDF from the one uniform of the position             */
     float ln_eps;      /* LayerNorm epsilon (reading A6: 1e-5)                                */
 } fv_config;
 
 /* Build a model object.
  *   weights [host]  n_weights fp32 values in this order, matrices row-major [out,in], y = Wx+b
- *       (Eq. 2, l.98-100): tok_emb[2,d_token]; per layer ln1_g[d] ln1_b[d] Wq[d,d] bq[d]
+ *       (Eq. 2, l.98-100): tok_emb[V,d_token] (V = vocab); per layer ln1_g[d] ln1_b[d] Wq[d,d] bq[d]
  *       Wk[d,d] bk[d] Wv[d,d] bv[d] (Wo[d,d] bo[d] iff has_wo) ln2_g[d] ln2_b[d] W1[4d,d]
- *       b1[4d] W2[d,4d] b2[d]; then head_W[2,d] head_b[2].  GEMM operands are rounded to bf16
+ *       b1[4d] W2[d,4d] b2[d]; then head_W[V,d] head_b[V].  GEMM operands are rounded to bf16
  *       once here; LayerNorm, biases, embeddings and the head stay fp32.
  *   mask_rowptr [host] N+1, mask_col [host] rowptr[N]: CSR in POSITION space (reading A11):
  *       row t lists the key positions A(t), ascending, unique, all <= t, last entry == t
@@ -79,12 +83,17 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
  *       (strict, compared in fp32; reading A10 replaces Categorical(p_t), l.359).
  *   spins  [device] [B,N] int8 out, values +-1 (l.361: sigma = 2 s - 1).
  *   logq   [device] [B] fp32 out: sum_t log p_t(s_t) (Alg. 1 l.9), accumulated in fp64.
- *   cond_p [device] [B,N] fp32 out or NULL: p_t(+1 | s_<t). */
+ *   cond_p [device] [B,N] fp32 out or NULL: p_t(+1 | s_<t).
+ * With vocab > 2 (patch tokens): `spins` receives the TOKEN of every position as an unsigned byte (0 .. vocab - 1;
+ * fv_tokens_to_spins unpacks them onto the lattice), drawn as the first k with u < p_0 + ... + p_k in token
+ * order (fp32 softmax over the `vocab` logits; the last token if rounding leaves u above the total); cond_p
+ * receives the probability of the drawn token. */
 int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, float* logq,
               float* cond_p, void* stream);
 
 /* Alg. 1: teacher-forced log q(s) of given configurations.
  *   spins [device] [B,N] int8 in (+-1; other values are undefined behaviour).
+ *   (vocab > 2: token ids as unsigned bytes, cond_p = probability of the given token.)
  *   logq, cond_p as in fv_sample.  Overwrites the model's KV pool and workspace: calls on one model
  *   must be ordered on one stream.  Enqueues 3 * n_layers + 1 kernels (layer-major tensor-core path) or
  *   one (chunked teacher forcing: d_model = 256 or has_wo). */
@@ -155,6 +164,13 @@ int fv_markov_mask(int32_t n, int64_t n_edges, const int32_t* edge_a, const int3
 
 /* Expected n_weights for a configuration (the layout above); < 0 on a bad shape. */
 int64_t fv_n_weights(const fv_config* cfg);
+
+/* Patch tokens -> lattice spins (SI I.D, l.603-605): bit k of token n of sample b is the spin (2 bit - 1, l.361) of
+ * lattice site site_index[n * P + k].
+ *   tokens [device] [B, n_tokens] unsigned bytes; site_index [device] [n_tokens * P] int32, a permutation of
+ *   0 .. n_tokens * P - 1 (P = spins per token <= 8); spins [device] [B, n_tokens * P] int8 out. */
+int fv_tokens_to_spins(int32_t B, int32_t n_tokens, int32_t P, const uint8_t* tokens, const int32_t* site_index,
+                       int8_t* spins, void* stream);
 
 /* Which of the two fv_sample kernels a batch of B samples takes on this model: "chain" (layer-pipelined clusters,
  * weights resident on chip: d_model = 128, 16-wide heads, no W_O, mask rows of <= 160 entries on average) or

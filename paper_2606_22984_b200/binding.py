@@ -17,13 +17,13 @@ _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.s
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
-           "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps", "fv_profile", "fv_sampler_kind"]
+           "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps", "fv_profile", "fv_sampler_kind", "fv_tokens_to_spins"]
 
 
 class FvConfig(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
                 ("n_sites", "n_layers", "d_model", "n_heads", "d_token", "ffn_mult", "has_wo", "act",
-                 "ln2_style", "max_batch")] + [("ln_eps", ctypes.c_float)]
+                 "ln2_style", "max_batch", "vocab")] + [("ln_eps", ctypes.c_float)]
 
 
 class FlashVanError(RuntimeError):
@@ -59,6 +59,7 @@ def lib() -> ctypes.CDLL:
         L.fv_lmc_sweeps.argtypes = [i32, i32, i32, vp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
         L.fv_overlap.argtypes = [i32, i32, vp, vp, vp, vp, vp]
         L.fv_profile.argtypes = [i32, vp, vp]
+        L.fv_tokens_to_spins.argtypes = [i32, i32, i32, vp, vp, vp, vp]
         L.fv_sampler_kind.argtypes = [vp, i32]
         L.fv_sampler_kind.restype = ctypes.c_char_p
         L.fv_markov_mask.argtypes = [i32, i64, vp, vp, i32, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(i32)]
@@ -106,7 +107,7 @@ def profile(enable: bool) -> dict:
 def make_config(w, max_batch: int) -> FvConfig:
     """`w` is any object with the Workload fields (n_sites, n_layers, d_model, ...)."""
     return FvConfig(w.n_sites, w.n_layers, w.d_model, w.n_heads, w.d_token, w.ffn_mult, w.has_wo, 0,
-                    w.ln2_style, max_batch, float(w.ln_eps))
+                    w.ln2_style, max_batch, int(getattr(w, "vocab", 2)), float(w.ln_eps))
 
 
 class Model:
@@ -228,6 +229,22 @@ def lmc_sweeps(spins, adj_rowptr, adj_col, adj_val, beta: float, exp_variates):
     _check(lib().fv_lmc_sweeps(B, N, ev.shape[1], spins.data_ptr(), rp.data_ptr(), col.data_ptr(), val.data_ptr(),
                                float(beta), ev.data_ptr(), acc.data_ptr(), _stream()), "fv_lmc_sweeps")
     return acc
+
+
+def tokens_to_spins(tokens, site_index):
+    """fv_tokens_to_spins: patch tokens (uint8 or int8 storage, [B, n_tokens] CUDA) -> lattice spins int8
+    [B, n_tokens * P]; site_index int32 [n_tokens, P] CUDA (bit k of token n is the spin of that lattice site)."""
+    if tokens.dtype not in (torch.uint8, torch.int8) or not tokens.is_cuda or not tokens.is_contiguous() or tokens.dim() != 2:
+        raise FlashVanError("tokens_to_spins: tokens must be a contiguous byte CUDA tensor [B, n_tokens]")
+    si = _dev(site_index, torch.int32)
+    B, n_tok = tokens.shape
+    if si.dim() != 2 or si.shape[0] != n_tok or not 1 <= si.shape[1] <= 8:
+        raise FlashVanError("tokens_to_spins: site_index must be [n_tokens, P] with P <= 8")
+    P = si.shape[1]
+    spins = torch.empty((B, n_tok * P), dtype=torch.int8, device=tokens.device)
+    _check(lib().fv_tokens_to_spins(B, n_tok, P, tokens.data_ptr(), si.data_ptr(), spins.data_ptr(), _stream()),
+           "fv_tokens_to_spins")
+    return spins
 
 
 def overlap(spins_a, spins_b, want_hist: bool = True):

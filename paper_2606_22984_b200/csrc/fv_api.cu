@@ -68,13 +68,15 @@ bool shape_ok(const fv_config* c) {
     if (c->n_heads <= 0 || c->d_model % c->n_heads) return false;
     const int dh = c->d_model / c->n_heads;
     const int key = c->d_model * 1000 + dh;
+    if (c->vocab != 0 && c->vocab != 2 && !((c->vocab == 16 || c->vocab == 256) && c->d_model <= 128 && !c->has_wo)) return false;
     return key == 32016 || key == 64016 || key == 64032 || key == 128016 || key == 128032 || key == 256064;
 }
 
 int64_t n_weights_of(const fv_config* c) {
     const int64_t d = c->d_model, f = 4 * d;
     const int64_t per = 2 * d + 3 * (d * d + d) + (c->has_wo ? d * d + d : 0) + 2 * d + f * d + f + d * f + d;
-    return 2 * (int64_t)c->d_token + c->n_layers * per + 2 * d + 2;
+    const int64_t V = c->vocab > 2 ? c->vocab : 2;
+    return V * (int64_t)c->d_token + c->n_layers * per + V * d + V;
 }
 
 uint16_t bf16_bits(float x) {
@@ -197,8 +199,9 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     std::vector<uint16_t> img((size_t)std::max(3 * d * KP, (f / HC) * (HC * KP + d * HC)));
     std::vector<Off> off(NL);
     const float* w = weights;
-    const size_t o_tok = A.put(w, sizeof(float) * 2 * cfg->d_token);
-    w += 2 * cfg->d_token;
+    const int V = cfg->vocab > 2 ? cfg->vocab : 2;
+    const size_t o_tok = A.put(w, sizeof(float) * V * cfg->d_token);
+    w += (size_t)V * cfg->d_token;
     std::vector<uint16_t> pk((size_t)f * d);
     std::vector<float> tmp((size_t)3 * d * d), tb(3 * d);
     for (int l = 0; l < NL; ++l) {
@@ -245,8 +248,10 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     }
     std::vector<float> wd(d);
     for (int i = 0; i < d; ++i) wd[i] = w[d + i] - w[i];            // head_W[1] - head_W[0]
-    const float bd = w[2 * d + 1] - w[2 * d];
+    const float bd = w[(size_t)V * d + 1] - w[(size_t)V * d];
     const size_t o_wd = A.put(wd.data(), 4 * d);
+    const size_t o_hw = A.put(w, sizeof(float) * (size_t)V * d);
+    const size_t o_hb = A.put(w + (size_t)V * d, sizeof(float) * V);
     const size_t o_pos = A.put(posemb, sizeof(float) * (size_t)N * (d - cfg->d_token));
     const size_t o_rp = A.put(mask_rowptr, sizeof(int32_t) * (N + 1));
     const size_t o_col = A.put(mask_col, sizeof(int32_t) * (size_t)mask_rowptr[N]);
@@ -326,6 +331,9 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.posemb = (const float*)(base + o_pos);
     D.head_wd = (const float*)(base + o_wd);
     D.head_bd = bd;
+    D.vocab = V;
+    D.head_w = (const float*)(base + o_hw);
+    D.head_b = (const float*)(base + o_hb);
     D.mask_rowptr = (const int32_t*)(base + o_rp);
     D.mask_col = (const int32_t*)(base + o_col);
     D.chunk_ptr = (const int32_t*)(base + o_cp);
@@ -472,6 +480,7 @@ int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float*
     if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
     if (int rc = wrong_device(m)) return rc;
     const char* force = std::getenv("FLASHVAN_LOGPROB");          // "chunked": the persistent teacher-forcing kernel
+    if (m->dev.vocab > 2) force = nullptr;                         // (one spin per token only)
     if (!(force && std::strcmp(force, "chunked") == 0)) {
         int n_launch = 0;
         cudaError_t e2 = fv_launch_logprob_tc(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B, spins, logq,
@@ -520,6 +529,16 @@ int fv_free_energy(int32_t B, const float* E, const float* logq, double temperat
     if (B <= 0) return fail(FV_ERR_BAD_ARG, "B must be positive");
     cudaError_t e = fv_launch_free_energy(B, E, logq, temperature, out, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "fv_free_energy launch");
+    g_launches++;
+    return FV_OK;
+}
+
+int fv_tokens_to_spins(int32_t B, int32_t n_tokens, int32_t P, const uint8_t* tokens, const int32_t* site_index,
+                       int8_t* spins, void* stream) {
+    if (!tokens || !site_index || !spins) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0 || n_tokens <= 0 || P <= 0 || P > 8) return fail(FV_ERR_BAD_ARG, "B, n_tokens must be positive and 1 <= P <= 8");
+    cudaError_t e = fv_launch_tokens_to_spins(B, n_tokens, P, tokens, site_index, spins, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fv_tokens_to_spins launch");
     g_launches++;
     return FV_OK;
 }

@@ -670,7 +670,7 @@ static int chain_clusters(int n_layers) {
 // (d = 128 with 16-wide heads, no W_O, at most 8 layers, batch small enough for 16 micro-batches of 16 per
 // chain): the caller then uses the streaming kernel of fv_decode.cu.
 static bool chain_geometry(const FvModelDev& m, int d_model, int d_head, int B, ChainArgs& a) {
-    if (d_model != D || d_head != DH || m.has_wo || m.n_layers > 8 || !m.layer[0].img_ffn || !m.layer[0].img_qkv)
+    if (d_model != D || d_head != DH || m.has_wo || m.vocab > 2 || m.n_layers > 8 || !m.layer[0].img_ffn || !m.layer[0].img_qkv)
         return false;
     const int C = chain_clusters(m.n_layers);
     if (C <= 0) return false;

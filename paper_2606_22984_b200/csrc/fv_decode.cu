@@ -691,6 +691,71 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
 
                 }
             }
+            // ---- patch tokens (SI I.D, l.603-605): V-way softmax head, token = first k with u < p_0 + .. + p_k ----
+            if (m.vocab > 2) {
+                const int V = m.vocab;
+                for (int r = warp; r < R; r += NWC) {
+                    if (r >= n_own) continue;
+                    const int b = b_first + r;
+                    // lane owns tokens lane, lane + 32, ...: logits, then everything in token order
+                    float z[8];
+                    float mx = -INFINITY;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int k = lane + 32 * i;
+                        z[i] = -INFINITY;
+                        if (k < V) {
+                            const float4* wr = reinterpret_cast<const float4*>(m.head_w + (size_t)k * D);
+                            float acc = __ldg(m.head_b + k);
+#pragma unroll 4
+                            for (int f4 = 0; f4 < D / 4; ++f4) {
+                                const float4 wv = __ldg(wr + f4);
+                                const float4 hv = *reinterpret_cast<const float4*>(sh_h + r * HS + f4 * 4);
+                                acc += hv.x * wv.x + hv.y * wv.y + hv.z * wv.z + hv.w * wv.w;
+                            }
+                            z[i] = acc;
+                            mx = fmaxf(mx, acc);
+                        }
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+                    float e[8], mine = 0.f;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) { e[i] = lane + 32 * i < V ? expf(z[i] - mx) : 0.f; mine += e[i]; }
+                    const float S = warp_sum(mine);
+                    // running sums in token order: block i (tokens 32 i .. 32 i + 31) after the blocks before it
+                    const float target = sh_u[r] * S;               // u < cdf_k  <=>  u S < e_0 + .. + e_k
+                    float carry = 0.f;
+                    int tok = V - 1;
+                    bool found = false;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        if (32 * i >= V) break;
+                        float pre = e[i];                            // inclusive scan over the lanes
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const float up = __shfl_up_sync(0xffffffffu, pre, o);
+                            if (lane >= o) pre += up;
+                        }
+                        pre += carry;
+                        const unsigned hit = __ballot_sync(0xffffffffu, lane + 32 * i < V && target < pre);
+                        if (!found && hit) { tok = 32 * i + __ffs(hit) - 1; found = true; }
+                        carry = __shfl_sync(0xffffffffu, pre, 31);
+                    }
+                    // the drawn token's logit and weight live in lane tok % 32, slot tok / 32
+                    float zt = 0.f, et = 0.f;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) if (i == (tok >> 5)) { zt = z[i]; et = e[i]; }
+                    zt = __shfl_sync(0xffffffffu, zt, tok & 31);
+                    et = __shfl_sync(0xffffffffu, et, tok & 31);
+                    if (lane == 0) {
+                        a.spins_out[(size_t)b * N + t] = (int8_t)(uint8_t)tok;
+                        sh_tok[r] = tok;
+                        sh_logp[r] = (zt - mx) - logf(S);
+                        if (a.cond_p) a.cond_p[(size_t)b * N + t] = et / S;
+                    }
+                }
+            } else
             // ---- output head: p(+1) = softmax(z)[1] = sigmoid(z1 - z0) (Alg. 2 l.20-22) -----
             for (int r = warp; r < R; r += NWC) {
                 if (r >= n_own) continue;

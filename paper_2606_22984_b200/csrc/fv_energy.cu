@@ -340,6 +340,24 @@ cudaError_t fv_launch_lmc(int B, int N, int n_sweeps, int8_t* spins, const int32
     return cudaGetLastError();
 }
 
+// Patch tokens -> lattice spins: one thread per (sample, token), P byte stores.
+__global__ void tokens_to_spins_kernel(int B, int n_tokens, int P, const uint8_t* __restrict__ tokens,
+                                       const int32_t* __restrict__ site_index, int8_t* __restrict__ spins) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)B * n_tokens) return;
+    const int n = (int)(i % n_tokens);
+    const long long b = i / n_tokens;
+    const unsigned tok = tokens[i];
+    for (int k = 0; k < P; ++k) spins[b * n_tokens * P + __ldg(site_index + n * P + k)] = ((tok >> k) & 1u) ? 1 : -1;
+}
+
+cudaError_t fv_launch_tokens_to_spins(int B, int n_tokens, int P, const uint8_t* tokens, const int32_t* site_index,
+                                      int8_t* spins, cudaStream_t s) {
+    const long long n = (long long)B * n_tokens;
+    tokens_to_spins_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(B, n_tokens, P, tokens, site_index, spins);
+    return cudaGetLastError();
+}
+
 cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out, cudaStream_t s) {
     free_energy_kernel<<<1, 1024, 0, s>>>(B, E, logq, T, out);
     return cudaGetLastError();

@@ -44,6 +44,9 @@ struct FvModelDev {
     const float* posemb;    // [N, d - d_token]
     const float* head_wd;   // [d]  = head_W[1] - head_W[0]   (softmax over 2 logits == sigmoid)
     float head_bd;          //      = head_b[1] - head_b[0]
+    int32_t vocab;          // 2, or 16 / 256 with patch tokens: then the V-way head below is used instead
+    const float* head_w;    // [vocab, d] fp32
+    const float* head_b;    // [vocab]
     const int32_t* mask_rowptr;
     const int32_t* mask_col;
     // KV ring copy plan of fv_decode.cu (derived from the mask at fv_create_model): row t minus its own
@@ -120,6 +123,8 @@ cudaError_t fv_launch_energy_dense(int B, int N, const int8_t* spins, const floa
 cudaError_t fv_launch_free_energy(int B, const float* E, const float* logq, double T, double* out,
                                   cudaStream_t s);
 
+cudaError_t fv_launch_tokens_to_spins(int B, int n_tokens, int P, const uint8_t* tokens, const int32_t* site_index,
+                                      int8_t* spins, cudaStream_t s);
 cudaError_t fv_launch_overlap(int B, int N, const int8_t* sa, const int8_t* sc, int32_t* dot, int32_t* hist,
                               cudaStream_t s);
 

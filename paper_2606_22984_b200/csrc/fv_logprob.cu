@@ -131,7 +131,7 @@ __device__ __forceinline__ uint32_t gelu_erfc_x2(float x0, float x1) {
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
 
 struct LpArgs {
-    int32_t B, N, NL, layer, d_token, ln2_style;
+    int32_t B, N, NL, layer, d_token, ln2_style, vocab;
     float ln_eps;
     long long M;                    // B * N rows
     const int8_t* spins;            // [B, N]
@@ -198,7 +198,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
             if (gi < a.M) {
                 if (a.layer == 0) {                 // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
                     const int t = (int)(gi % a.N);
-                    const int tok = t > 0 ? (a.spins[gi - 1] > 0 ? 1 : 0) : 0;
+                    const int tok = t == 0 ? 0 : (a.vocab > 2 ? (int)(uint8_t)a.spins[gi - 1] : (a.spins[gi - 1] > 0 ? 1 : 0));
 #pragma unroll
                     for (int k = 0; k < NV; ++k) {
                         float e[4];
@@ -884,6 +884,62 @@ __global__ void __launch_bounds__(256) lp_head_kernel(const __grid_constant__ Lp
     }
 }
 
+// Patch tokens (SI I.D, l.603-605): V-way softmax head, log p of the given token; one warp per position, lane owns
+// tokens lane, lane + 32, ...; per-sample fp64 sum in the same fixed order as lp_head_kernel.
+template <int D>
+__global__ void __launch_bounds__(256) lp_head_tok_kernel(const __grid_constant__ LpArgs a, const float* __restrict__ head_w,
+                                                          const float* __restrict__ head_b, float* __restrict__ logq,
+                                                          float* __restrict__ cond_p) {
+    __shared__ double red[8];
+    __shared__ __align__(16) float sh_row[8][D];
+    const int b = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int V = a.vocab;
+    double acc = 0.0;
+    for (int t = warp; t < a.N; t += 8) {
+        const long long gi = (long long)b * a.N + t;
+        for (int f = lane; f < D; f += 32) sh_row[warp][f] = a.h[gi * D + f];
+        __syncwarp();
+        const int tok = (int)(uint8_t)a.spins[gi];
+        float mx = -INFINITY, zt = 0.f, z[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int k = lane + 32 * i;
+            z[i] = -INFINITY;
+            if (k < V) {
+                const float4* wr = reinterpret_cast<const float4*>(head_w + (size_t)k * D);
+                float d = __ldg(head_b + k);
+#pragma unroll 4
+                for (int f4 = 0; f4 < D / 4; ++f4) {
+                    const float4 wv = __ldg(wr + f4);
+                    const float4 hv = *reinterpret_cast<const float4*>(&sh_row[warp][f4 * 4]);
+                    d += hv.x * wv.x + hv.y * wv.y + hv.z * wv.z + hv.w * wv.w;
+                }
+                z[i] = d;
+                mx = fmaxf(mx, d);
+                if (k == tok) zt = d;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        float mine = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) mine += lane + 32 * i < V ? expf(z[i] - mx) : 0.f;
+        const float S = warp_sum(mine);
+        zt = __shfl_sync(0xffffffffu, zt, tok & 31);
+        const float lp = (zt - mx) - logf(S);
+        acc += (double)lp;
+        if (cond_p && lane == 0) cond_p[gi] = expf(zt - mx) / S;
+        __syncwarp();
+    }
+    if (lane == 0) red[warp] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < 8; ++i) s += red[i];
+        logq[b] = (float)s;
+    }
+}
+
 template <int D, int DH>
 cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* logq, float* cond_p, int n_sms,
                       cudaStream_t s) {
@@ -898,6 +954,7 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
     }
     LpArgs a{};
     a.B = B; a.N = m.n_sites; a.NL = m.n_layers; a.d_token = m.d_token; a.ln2_style = m.ln2_style; a.ln_eps = m.ln_eps;
+    a.vocab = m.vocab;
     a.M = (long long)B * m.n_sites;
     a.spins = spins; a.h = m.lp_h; a.q = m.lp_q; a.kv = m.kv; a.tok_emb = m.tok_emb; a.posemb = m.posemb;
     const long long n_tiles = (a.M + TM - 1) / TM;
@@ -926,7 +983,8 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
         fv_prof_end(FV_K_LP_FFN, s);
     }
     fv_prof_begin(FV_K_LP_HEAD, s);
-    lp_head_kernel<D><<<B, 256, 0, s>>>(a, m.head_wd, m.head_bd, logq, cond_p);
+    if (m.vocab > 2) lp_head_tok_kernel<D><<<B, 256, 0, s>>>(a, m.head_w, m.head_b, logq, cond_p);
+    else lp_head_kernel<D><<<B, 256, 0, s>>>(a, m.head_wd, m.head_bd, logq, cond_p);
     fv_prof_end(FV_K_LP_HEAD, s);
     return cudaGetLastError();
 }
