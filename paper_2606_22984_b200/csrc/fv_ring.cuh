@@ -101,15 +101,35 @@ __device__ __forceinline__ void st_release_s32(int* p, int v) {
     asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
 
+// Packed fp32 arithmetic of sm_100 (fma.rn.f32x2: two independent FMAs per instruction, operands in 64-bit registers).
+__device__ __forceinline__ uint64_t f2pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void f2unpack(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// the two bf16 of a 32-bit word as an fp32 pair (exact)
+__device__ __forceinline__ uint64_t bf2_to_f2(uint32_t w) { return f2pack(bf_lo(w), bf_hi(w)); }
+
 // Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
 // PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
 // with 128-bit shared loads and the matching 16 B of V; RPI = 32/LPR rows per iteration.
+// The phase is issue-bound (about 25 instructions per row and warp before, two thirds of them the
+// bf16 unpacking and the FMAs): scores and the P V update run on the packed fp32 pipe, even and odd
+// features in the two halves of a register pair, which takes a third of the FMA instructions out.
 template <int D, int DH, int CH>
 __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
                                              float& m, float& l, float (&acc)[8]) {
     constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
     constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
     const unsigned char* base = chunk + sub * 16;
+    const uint64_t q2[4] = {f2pack(q[0], q[1]), f2pack(q[2], q[3]), f2pack(q[4], q[5]), f2pack(q[6], q[7])};
+    uint64_t a2[4] = {f2pack(acc[0], acc[1]), f2pack(acc[2], acc[3]), f2pack(acc[4], acc[5]), f2pack(acc[6], acc[7])};
     for (int i0 = 0; i0 < rows; i0 += RPI * U) {
         uint4 kk[U], vv[U];
         bool ok[U];
@@ -125,10 +145,13 @@ __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int row
         float mx = m;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            float d = q[0] * bf_lo(kk[u].x) + q[1] * bf_hi(kk[u].x);
-            d += q[2] * bf_lo(kk[u].y) + q[3] * bf_hi(kk[u].y);
-            d += q[4] * bf_lo(kk[u].z) + q[5] * bf_hi(kk[u].z);
-            d += q[6] * bf_lo(kk[u].w) + q[7] * bf_hi(kk[u].w);
+            uint64_t d2 = ffma2(q2[0], bf2_to_f2(kk[u].x), 0ull);
+            d2 = ffma2(q2[1], bf2_to_f2(kk[u].y), d2);
+            d2 = ffma2(q2[2], bf2_to_f2(kk[u].z), d2);
+            d2 = ffma2(q2[3], bf2_to_f2(kk[u].w), d2);
+            float de, dodd;
+            f2unpack(d2, de, dodd);
+            float d = de + dodd;
 #pragma unroll
             for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
             s[u] = ok[u] ? d : -INFINITY;
@@ -137,18 +160,22 @@ __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int row
         const float corr = fast_exp2(m - mx);
         m = mx;
         l *= corr;
+        const uint64_t c2 = f2pack(corr, corr);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc[j] *= corr;
+        for (int j = 0; j < 4; ++j) a2[j] = ffma2(a2[j], c2, 0ull);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const float p = fast_exp2(s[u] - mx);
             l += p;
-            acc[0] += p * bf_lo(vv[u].x); acc[1] += p * bf_hi(vv[u].x);
-            acc[2] += p * bf_lo(vv[u].y); acc[3] += p * bf_hi(vv[u].y);
-            acc[4] += p * bf_lo(vv[u].z); acc[5] += p * bf_hi(vv[u].z);
-            acc[6] += p * bf_lo(vv[u].w); acc[7] += p * bf_hi(vv[u].w);
+            const uint64_t p2 = f2pack(p, p);
+            a2[0] = ffma2(p2, bf2_to_f2(vv[u].x), a2[0]);
+            a2[1] = ffma2(p2, bf2_to_f2(vv[u].y), a2[1]);
+            a2[2] = ffma2(p2, bf2_to_f2(vv[u].z), a2[2]);
+            a2[3] = ffma2(p2, bf2_to_f2(vv[u].w), a2[3]);
         }
     }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) f2unpack(a2[j], acc[2 * j], acc[2 * j + 1]);
 }
 
 // Consumer side of a ring chunk: wait until the producer has armed this round of the slot (a
