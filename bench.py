@@ -52,7 +52,7 @@ def sampler_source_hash():
     return h.hexdigest()[:16]
 
 
-def ncu_traffic(workload, batch):
+def ncu_traffic(workload, batch, kind="ring"):
     """DRAM and L2->SM bytes of the fv_sample launch from the committed ncu capture: the row of
     profiles/sampler_traffic.csv for this (workload, batch), quoted only if it was captured on the
     sampler sources as they are now.  Returns (dict or None, note)."""
@@ -60,7 +60,7 @@ def ncu_traffic(workload, batch):
     if not os.path.exists(path):
         return None, "no profiles/sampler_traffic.csv"
     rows = [r for r in csv.DictReader(l for l in open(path) if not l.startswith("#"))
-            if r["workload"] == workload and int(r["batch"]) == batch]
+            if r["workload"].split("_")[0] == workload and int(r["batch"]) == batch and ("chain" in r["kernel"]) == (kind == "chain")]
     if not rows:
         return None, f"no ncu capture of {workload} at batch {batch} in profiles/sampler_traffic.csv"
     r = rows[-1]
@@ -344,7 +344,7 @@ def run_ours(args):
         peak, tf_peak, peak_src = load_peaks()
         k_sample_ms = kernel_ms["sample"][0] / max(1, kernel_ms["sample"][1])      # library-side events, kernel only
         achieved = (rd + wr) * B / (k_sample_ms * 1e-3) / 1e9
-        traffic, traffic_note = ncu_traffic(w.name, B)
+        traffic, traffic_note = ncu_traffic(w.name, B, sampler_kind)
         ffn_ms = kernel_ms["lp_ffn"][0] / max(1, kernel_ms["lp_ffn"][1])
         ffn_flop = 2.0 * B * N * (w.d_model * 4 * w.d_model) * 2
         out = {
