@@ -172,9 +172,10 @@ int64_t fv_n_weights(const fv_config* cfg);
 int fv_tokens_to_spins(int32_t B, int32_t n_tokens, int32_t P, const uint8_t* tokens, const int32_t* site_index,
                        int8_t* spins, void* stream);
 
-/* Which of the two fv_sample kernels a batch of B samples takes on this model: "chain" (layer-pipelined clusters,
- * weights resident on chip: d_model = 128, 16-wide heads, no W_O, mask rows of <= 160 entries on average) or
- * "ring" (one CTA per sample group, weights streamed); "none" for bad arguments.  A static string. */
+/* Which fv_sample kernel a batch of B samples takes on this model: "ring-tc" (one CTA per sample group, KV rows and
+ * weights streamed through one shared-memory ring, projections on tcgen05: d_model = 128, 16-wide heads, no W_O),
+ * "ring" (the same with mma.sync projections: every other shape, or FLASHVAN_DECODE=ring), "chain" (layer-pipelined
+ * clusters with the weights resident on chip, FLASHVAN_DECODE=chain); "none" for bad arguments.  A static string. */
 const char* fv_sampler_kind(const fv_model* m, int32_t B);
 
 /* Per-kernel device times, for measurement (bench.py's GEMM roofline).  While switched on, the library brackets

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libflashvan.so")
-SOURCES = ["fv_forward.cu", "fv_decode.cu", "fv_chain.cu", "fv_logprob.cu", "fv_energy.cu", "fv_mask.cu", "fv_api.cu"]
+SOURCES = ["fv_forward.cu", "fv_decode.cu", "fv_decode_tc.cu", "fv_chain.cu", "fv_logprob.cu", "fv_energy.cu", "fv_mask.cu", "fv_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC"] + os.environ.get("FLASHVAN_NVCC_EXTRA", "").split()
 

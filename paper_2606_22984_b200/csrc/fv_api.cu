@@ -56,6 +56,16 @@ bool wants_chain(const fv_model* m) {
     return false;             // opt-in until it beats the streaming kernel
 }
 
+// The streaming sampler with tcgen05 projections (fv_decode_tc.cu) is the default where it exists (d = 128, 16-wide heads,
+// no W_O); FLASHVAN_DECODE=ring keeps the mma.sync kernel of fv_decode.cu for comparison.
+// nt = n8-tiles of samples per CTA: with <= 8 samples per CTA the separate MMA / epilogue round trips of the tcgen05 path
+// cost more than they save (cfg5: 292 vs 252 ms), from 9 samples per CTA on it wins (cfg4, 28 per CTA: 83.6 vs 91.0 ms).
+bool wants_tc(const fv_model* m, int nt) {
+    const char* dmode = std::getenv("FLASHVAN_DECODE");
+    if (dmode && *dmode) return std::strcmp(dmode, "tc") == 0;
+    return nt >= 2 && m->cfg.d_model == 128 && m->cfg.d_model / m->cfg.n_heads == 16 && !m->cfg.has_wo;
+}
+
 int cuda_fail(cudaError_t e, const char* what) {
     return fail(e == cudaErrorMemoryAllocation ? FV_ERR_OOM : FV_ERR_CUDA,
                 std::string(what) + ": " + cudaGetErrorString(e));
@@ -192,7 +202,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     m->mean_nnz = (double)mask_rowptr[N] / N;
     m->device = dev;
     Arena A;
-    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn; };
+    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn, img_w1t; };
     const bool lp_tc = !cfg->has_wo && (d == 32 || d == 64 || d == 128);   // fv_logprob.cu path
     const int KP = d < 64 ? 64 : d;
     const int HC = FV_LP_HC;
@@ -214,7 +224,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         }
         pack_mma_a(tmp.data(), 3 * d, d, pk.data());
         o.wqkv = A.put(pk.data(), (size_t)3 * d * d * 2);
-        o.img_qkv = o.img_ffn = 0;
+        o.img_qkv = o.img_ffn = o.img_w1t = 0;
         if (lp_tc) {
             fv_pack_sw128(tmp.data(), 3 * d, d, d, KP, img.data());
             o.img_qkv = A.put(img.data(), (size_t)3 * d * KP * 2);
@@ -238,6 +248,11 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
                 fv_pack_sw128(W2 + (size_t)j * HC, d, HC, f, HC, img.data() + j * per + (size_t)HC * KP);
             }
             o.img_ffn = A.put(img.data(), (size_t)(f / HC) * per * 2);
+            o.img_w1t = 0;
+            if (d == 128) {                           // fv_decode_tc.cu: the same W1 as [128 rows x 64 K] tiles, M-tile-major
+                for (int mt = 0; mt < f / 128; ++mt) fv_pack_sw128(W1 + (size_t)mt * 128 * d, 128, d, d, d, img.data() + (size_t)mt * 128 * d);
+                o.img_w1t = A.put(img.data(), (size_t)f * d * 2);
+            }
         }
         w += (size_t)f * d;
         o.w1 = A.put(pk.data(), (size_t)f * d * 2);
@@ -361,6 +376,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         L.ln2_g = (const float*)(base + o.ln2g); L.ln2_b = (const float*)(base + o.ln2b);
         L.img_qkv = lp_tc ? base + o.img_qkv : nullptr;
         L.img_ffn = lp_tc ? base + o.img_ffn : nullptr;
+        L.img_w1t = (lp_tc && d == 128) ? base + o.img_w1t : nullptr;
     }
     *out = m;
     return FV_OK;
@@ -462,8 +478,12 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
     const char* dm = std::getenv("FLASHVAN_DECODE");
     const int cluster = dm && std::strcmp(dm, "cluster") == 0 && !m->cfg.has_wo;
     fv_prof_begin(FV_K_SAMPLE, (cudaStream_t)stream);
-    cudaError_t e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, m->n_sms, cluster,
-                                     (cudaStream_t)stream);
+    cudaError_t e = cudaErrorNotSupported;
+    if (wants_tc(m, nt)) e = fv_launch_decode_tc(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, m->n_sms, (cudaStream_t)stream);
+    if (e == cudaErrorNotSupported) {
+        (void)cudaGetLastError();
+        e = fv_launch_decode(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, nt, a, m->n_sms, cluster, (cudaStream_t)stream);
+    }
     fv_prof_end(FV_K_SAMPLE, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "fv_sample launch");
     g_launches++;
@@ -472,7 +492,10 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
 
 const char* fv_sampler_kind(const fv_model* m, int32_t B) {
     if (!m || B <= 0) return "none";
-    return wants_chain(m) && fv_chain_supported(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B) ? "chain" : "ring";
+    if (wants_chain(m) && fv_chain_supported(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B)) return "chain";
+    int S, nt, ng, grid;
+    sample_geometry(B, m->n_sms, &S, &nt, &ng, &grid);
+    return wants_tc(m, nt) && m->cfg.d_model == 128 && m->cfg.d_model / m->cfg.n_heads == 16 && !m->cfg.has_wo ? "ring-tc" : "ring";
 }
 
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {

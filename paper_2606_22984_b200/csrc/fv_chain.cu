@@ -105,65 +105,6 @@ __device__ __forceinline__ void st_peer_s32(uint32_t raddr, int v) {
     asm volatile("st.shared::cluster.s32 [%0], %1;\n" ::"r"(raddr), "r"(v) : "memory");
 }
 
-// ---- tcgen05 pieces not in fv_umma.cuh: A operand from tensor memory, TMEM stores, narrow loads ---------
-__device__ __forceinline__ void mma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n"
-        ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void mma_bf16_ss(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint4& v) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};\n"
-                 ::"r"(taddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-template <int NC>
-__device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, float (&v)[NC]) {
-    static_assert(NC == 8 || NC == 16, "8 or 16 columns");
-    uint32_t r[16];
-    if constexpr (NC == 16) {
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-            "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
-            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-            : "r"(taddr));
-    } else {
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
-            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-            : "r"(taddr));
-    }
-    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < NC; ++i) v[i] = __uint_as_float(r[i]);
-}
-
-// LayerNorm of one fp32 row in shared memory (reading A6), one warp per row, written as row r of the
-// [16 x 128] K-major SWIZZLE_128B B tile (two K-blocks of 16 rows x 128 B).
-__device__ __forceinline__ void ln_row_btile(float* hrow, const float* __restrict__ gam, const float* __restrict__ bet,
-                                             float eps, bool replace, unsigned char* btile, int r, int lane) {
-    const float4 x = *reinterpret_cast<const float4*>(hrow + lane * 4);
-    const float mean = warp_sum(x.x + x.y + x.z + x.w) * (1.0f / D);
-    const float d0 = x.x - mean, d1 = x.y - mean, d2 = x.z - mean, d3 = x.w - mean;
-    const float rstd = rsqrtf(warp_sum(d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3) * (1.0f / D) + eps);
-    const float4 g = __ldg(reinterpret_cast<const float4*>(gam) + lane), b = __ldg(reinterpret_cast<const float4*>(bet) + lane);
-    const float y0 = d0 * rstd * g.x + b.x, y1 = d1 * rstd * g.y + b.y, y2 = d2 * rstd * g.z + b.z, y3 = d3 * rstd * g.w + b.w;
-    const int i0 = lane * 4, kb = i0 >> 6, c = (i0 & 63) >> 3;
-    uint2 pk;
-    pk.x = pack_bf16(y0, y1);
-    pk.y = pack_bf16(y2, y3);
-    *reinterpret_cast<uint2*>(btile + kb * 2048 + umma::sw128_chunk(r, c) + (i0 & 7) * 2) = pk;
-    if (replace) *reinterpret_cast<float4*>(hrow + lane * 4) = make_float4(y0, y1, y2, y3);
-}
-
 template <int RMAX>
 __global__ void __launch_bounds__(NTHREADS, 1)
 fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ ChainArgs a) {
@@ -336,7 +277,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
 #pragma unroll
                 for (int c = 0; c < 8; ++c) {
                     const uint4 v = __ldg(reinterpret_cast<const uint4*>(img + (size_t)kb * rows_per_kb * 128 + umma::sw128_chunk(rr, c)));
-                    tmem_st4(tbase + kb * 32 + c * 4, v);
+                    umma::tmem_st4(tbase + kb * 32 + c * 4, v);
                 }
         }
         asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory");
@@ -382,7 +323,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             float* sh_u = sh_ubuf + buf * RMAX;
             if (last && tid < RMAX) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
             // ---- LN1 (Alg. 2 l.12) -> B tile ----------------------------------------------------------------------
-            for (int r = warp; r < n_own; r += NWC) ln_row_btile(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_bact, r, lane);
+            for (int r = warp; r < n_own; r += NWC) ln_row_btile<16>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_bact, r, lane);
             umma::fence_smem_to_async();
             cbar();
             // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13): D[feature, sample] = W_qkv[tile] . a^T -------------------------
@@ -393,7 +334,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                     umma::fence_after_sync();
 #pragma unroll
                     for (int ks = 0; ks < 8; ++ks)
-                        mma_bf16_ts(tm + TC_ACC + warp * 16, tm + TC_WQKV + warp * 64 + ks * 8,
+                        umma::mma_bf16_ts(tm + TC_ACC + warp * 16, tm + TC_WQKV + warp * 64 + ks * 8,
                                     bd_act + (uint64_t)(((ks >> 2) * 2048 + (ks & 3) * 32) >> 4), idesc, ks != 0);
                     umma::commit(bar_mma);
                 } else {
@@ -405,7 +346,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             if (warp < 12) {
                 const int mt = warp >> 2, fl = (warp & 3) * 32 + lane;
                 float v[NC];
-                tmem_ld_cols<NC>(tm + ((uint32_t)((warp & 3) * 32) << 16) + TC_ACC + mt * 16, v);
+                umma::tmem_ld_cols<NC>(tm + ((uint32_t)((warp & 3) * 32) << 16) + TC_ACC + mt * 16, v);
                 const float bias = __ldg(L.bqkv + mt * D + fl);
                 if (mt == 0) {
 #pragma unroll
@@ -509,7 +450,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                 cbar();
             }
             // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) -> B tile ------------------------------------------
-            for (int r = warp; r < n_own; r += NWC) ln_row_btile(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_bact, r, lane);
+            for (int r = warp; r < n_own; r += NWC) ln_row_btile<16>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_bact, r, lane);
             umma::fence_smem_to_async();
             cbar();
             // ---- FFN up-projection + exact GELU -> hidden B tile [16 x 512] ---------------------------------------
@@ -517,7 +458,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                 umma::fence_after_sync();
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks)
-                    mma_bf16_ts(tm + TC_ACC + warp * 16, tm + TC_W1 + warp * 64 + ks * 8,
+                    umma::mma_bf16_ts(tm + TC_ACC + warp * 16, tm + TC_W1 + warp * 64 + ks * 8,
                                 bd_act + (uint64_t)(((ks >> 2) * 2048 + (ks & 3) * 32) >> 4), idesc, ks != 0);
                 umma::commit(bar_mma);
             }
@@ -526,7 +467,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             {
                 const int mt = warp >> 2, jl = (warp & 3) * 32 + lane, j = mt * 128 + jl;     // hidden unit
                 float v[NC];
-                tmem_ld_cols<NC>(tm + ((uint32_t)((warp & 3) * 32) << 16) + TC_ACC + mt * 16, v);
+                umma::tmem_ld_cols<NC>(tm + ((uint32_t)((warp & 3) * 32) << 16) + TC_ACC + mt * 16, v);
                 const float b1 = __ldg(L.b1 + j);
                 unsigned char* dst = sh_bhid + (j >> 6) * 2048 + (j & 7) * 2;
                 const int c = (j & 63) >> 3;
@@ -544,7 +485,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
 #pragma unroll
                 for (int k8 = 0; k8 < 8; ++k8) {
                     const int ks = warp * 8 + k8;
-                    mma_bf16_ss(tm + TC_ACC + warp * 16, ad_w2 + (uint64_t)(((ks >> 2) * 16384 + (ks & 3) * 32) >> 4),
+                    umma::mma_bf16_ss_u(tm + TC_ACC + warp * 16, ad_w2 + (uint64_t)(((ks >> 2) * 16384 + (ks & 3) * 32) >> 4),
                                 bd_hid + (uint64_t)(((ks >> 2) * 2048 + (ks & 3) * 32) >> 4), idesc, k8 != 0);
                 }
                 umma::commit(bar_mma);
@@ -554,11 +495,11 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
             if (warp < 4) {
                 const int f = warp * 32 + lane;
                 float v[NC];
-                tmem_ld_cols<NC>(tm + ((uint32_t)(warp * 32) << 16) + TC_ACC, v);
+                umma::tmem_ld_cols<NC>(tm + ((uint32_t)(warp * 32) << 16) + TC_ACC, v);
 #pragma unroll
                 for (int part = 1; part < 4; ++part) {
                     float v2[NC];
-                    tmem_ld_cols<NC>(tm + ((uint32_t)(warp * 32) << 16) + TC_ACC + part * 16, v2);
+                    umma::tmem_ld_cols<NC>(tm + ((uint32_t)(warp * 32) << 16) + TC_ACC + part * 16, v2);
 #pragma unroll
                     for (int s = 0; s < NC; ++s) v[s] += v2[s];
                 }

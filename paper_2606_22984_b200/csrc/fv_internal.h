@@ -33,7 +33,8 @@ struct FvLayerDev {
     const float *ln1_g, *ln1_b, *ln2_g, *ln2_b;
     // fv_logprob.cu: pre-swizzled (SWIZZLE_128B, K-major) bf16 images, copied verbatim into shared memory
     const unsigned char* img_qkv;   // [3d rows x KP]
-    const unsigned char* img_ffn;   // per 128-column hidden chunk j: W1_j [128 x KP] | W2_j [d x 128]
+    const unsigned char* img_ffn;   // per 64-column hidden chunk j: W1_j [64 x KP] | W2_j [d x 64]
+    const unsigned char* img_w1t;   // fv_decode_tc.cu (d = 128): W1 per 128-row M-tile and 64-column K-block, [128 x 64] tiles of 16 KB
 };
 
 struct FvModelDev {
@@ -110,6 +111,8 @@ cudaError_t fv_launch_forward(const FvModelDev& m, int d_model, int d_head, int 
 size_t fv_forward_smem_bytes(int d_model, int nt);
 cudaError_t fv_launch_decode(const FvModelDev& m, int d_model, int d_head, int nt,
                              const FvForwardArgs& a, int n_sms, int cluster, cudaStream_t s);
+cudaError_t fv_launch_decode_tc(const FvModelDev& m, int d_model, int d_head, int nt, const FvForwardArgs& a, int n_sms,
+                                cudaStream_t s);
 bool fv_chain_supported(const FvModelDev& m, int d_model, int d_head, int B);
 cudaError_t fv_launch_chain(const FvModelDev& m, int d_model, int d_head, const FvForwardArgs& a, cudaStream_t s);
 cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,

@@ -93,41 +93,6 @@ __device__ __forceinline__ void ln8_to_tile(float4 (&x)[D / 32], const float* __
     }
 }
 
-// erfc-based exact-GELU with ONE special-function instruction: Phi(-|x|) = 0.5 erfc(|x| / sqrt 2) = 2^P(|x|) with a
-// degree-6 polynomial P fitted on [0, 10] (max |error| of the GELU 5e-8 in exact arithmetic, 5e-7 in fp32 --
-// below the bf16 rounding of the result by four orders of magnitude); gelu(x) = max(x, 0) - |x| Phi(-|x|).
-// P(a) = -0.9999930605 - 1.151201707 a - 0.4587709584 a^2 - 0.05341212449 a^3 + 8.080729771e-3 a^4
-//        - 7.692237508e-4 a^5 + 3.309327859e-5 a^6, |x| clamped to 10 (beyond it Phi(-|x|) < 1e-23).
-// Two of them at once on the packed fp32 pipe (fma.rn.f32x2: one instruction, two FMAs) -> one bf16x2 word.
-__device__ __forceinline__ uint64_t f2pack(float lo, float hi) {
-    uint64_t r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
-    uint64_t d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ uint32_t gelu_erfc_x2(float x0, float x1) {
-    const float a0 = fminf(fabsf(x0), 10.0f), a1 = fminf(fabsf(x1), 10.0f);
-    const uint64_t ax = f2pack(a0, a1);
-    uint64_t p = ffma2(f2pack(3.309327859e-05f, 3.309327859e-05f), ax, f2pack(-7.692237508e-04f, -7.692237508e-04f));
-    p = ffma2(p, ax, f2pack(8.080729771e-03f, 8.080729771e-03f));
-    p = ffma2(p, ax, f2pack(-5.341212449e-02f, -5.341212449e-02f));
-    p = ffma2(p, ax, f2pack(-4.587709584e-01f, -4.587709584e-01f));
-    p = ffma2(p, ax, f2pack(-1.151201707e+00f, -1.151201707e+00f));
-    p = ffma2(p, ax, f2pack(-9.999930605e-01f, -9.999930605e-01f));
-    float p0, p1, e0, e1;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(p0), "=f"(p1) : "l"(p));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e0) : "f"(p0));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e1) : "f"(p1));
-    const uint64_t g = ffma2(f2pack(-a0, -a1), f2pack(e0, e1), f2pack(fmaxf(x0, 0.f), fmaxf(x1, 0.f)));
-    float g0, g1;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(g0), "=f"(g1) : "l"(g));
-    return pack_bf16(g0, g1);
-}
-
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
 
 struct LpArgs {

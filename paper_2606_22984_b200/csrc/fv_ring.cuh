@@ -5,6 +5,7 @@
 // with the rows of one ring chunk (Eq. 3).
 #pragma once
 #include "fv_device.cuh"
+#include "fv_umma.cuh"
 
 namespace fvring {
 using namespace fvdev;
@@ -101,21 +102,6 @@ __device__ __forceinline__ void st_release_s32(int* p, int v) {
     asm volatile("st.release.cta.shared.s32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
 
-// Packed fp32 arithmetic of sm_100 (fma.rn.f32x2: two independent FMAs per instruction, operands in 64-bit registers).
-__device__ __forceinline__ uint64_t f2pack(float lo, float hi) {
-    uint64_t r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void f2unpack(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
-    uint64_t d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-// the two bf16 of a 32-bit word as an fp32 pair (exact)
-__device__ __forceinline__ uint64_t bf2_to_f2(uint32_t w) { return f2pack(bf_lo(w), bf_hi(w)); }
-
 // Online-softmax update of one query row with the `rows` KV rows of one ring chunk (Eq. 3,
 // PAPER.md:102).  Lane layout as attend_range (fv_device.cuh): LPR = D/8 lanes cover one K row
 // with 128-bit shared loads and the matching 16 B of V; RPI = 32/LPR rows per iteration.
@@ -176,6 +162,26 @@ __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int row
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) f2unpack(a2[j], acc[2 * j], acc[2 * j + 1]);
+}
+
+// LayerNorm of one fp32 row of 128 features in shared memory (reading A6), one warp per row, written as row r of
+// the [NB x 128] K-major SWIZZLE_128B B tile of a swap-AB tcgen05 GEMM (two K-blocks of NB rows x 128 B).
+template <int NB>
+__device__ __forceinline__ void ln_row_btile(float* hrow, const float* __restrict__ gam, const float* __restrict__ bet,
+                                             float eps, bool replace, unsigned char* btile, int r, int lane) {
+    constexpr int DD = 128;
+    const float4 x = *reinterpret_cast<const float4*>(hrow + lane * 4);
+    const float mean = warp_sum(x.x + x.y + x.z + x.w) * (1.0f / DD);
+    const float d0 = x.x - mean, d1 = x.y - mean, d2 = x.z - mean, d3 = x.w - mean;
+    const float rstd = rsqrtf(warp_sum(d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3) * (1.0f / DD) + eps);
+    const float4 g = __ldg(reinterpret_cast<const float4*>(gam) + lane), b = __ldg(reinterpret_cast<const float4*>(bet) + lane);
+    const float y0 = d0 * rstd * g.x + b.x, y1 = d1 * rstd * g.y + b.y, y2 = d2 * rstd * g.z + b.z, y3 = d3 * rstd * g.w + b.w;
+    const int i0 = lane * 4, kb = i0 >> 6, c = (i0 & 63) >> 3;
+    uint2 pk;
+    pk.x = pack_bf16(y0, y1);
+    pk.y = pack_bf16(y2, y3);
+    *reinterpret_cast<uint2*>(btile + kb * (NB * 128) + umma::sw128_chunk(r, c) + (i0 & 7) * 2) = pk;
+    if (replace) *reinterpret_cast<float4*>(hrow + lane * 4) = make_float4(y0, y1, y2, y3);
 }
 
 // Consumer side of a ring chunk: wait until the producer has armed this round of the slot (a

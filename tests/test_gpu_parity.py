@@ -277,6 +277,41 @@ def test_chain_sampler(case, monkeypatch):
     model.close()
 
 
+@pytest.mark.parametrize("case,B", [("sk_causal_4l", 41), ("ea3d_4l", 150), ("ea2d_6l_B300", 300), ("ea2d_6l_B300", 3000),
+                                    ("ea2d_2l_16_per_microbatch", 2300), ("ln2_style_1", 45)])
+def test_tcgen05_streaming_sampler(case, B, monkeypatch):
+    """FLASHVAN_DECODE=tc: fv_decode_tc.cu (the streaming sampler with its projections on tcgen05, weight tiles read by
+    the tensor core straight from the ring) on 1 to 32 samples per CTA, against the oracle like the default kernels;
+    it is the default from 9 samples per CTA on."""
+    base, kw, _ = CHAIN_CASES[case]
+    w = dataclasses.replace(W.CONFIGS[base], **kw)
+    model, weights, posemb, rp, col = build(w, B)
+    assert model.sampler_kind(B) == ("ring-tc" if B > 8 * torch.cuda.get_device_properties(0).multi_processor_count else "ring")
+    monkeypatch.setenv("FLASHVAN_DECODE", "tc")
+    assert model.sampler_kind(B) == "ring-tc"
+    n = min(B, 300)
+    idx = np.unique(np.linspace(0, B - 1, n).astype(np.int64))
+    u = W.make_uniforms(w, B)
+    spins_g, lq_g, cp_g = model.sample(dev(u), want_cond_p=True)
+    s = spins_g.cpu().numpy()[idx]
+    lq_o, cp_o = O.log_prob(w, weights, posemb, rp, col, s)
+    cp_s = cp_g.cpu().numpy().astype(np.float64)[idx]
+    assert np.abs(cp_s - cp_o).max() <= TOL_P
+    uu = u[idx].astype(np.float64)
+    mism = s != np.where(uu < cp_o, 1, -1)
+    tie = np.abs(uu - cp_o) < TOL_P
+    assert not (mism & ~tie).any()
+    picked = np.where(s > 0, cp_o, 1 - cp_o)
+    assert (np.abs(lq_g.cpu().numpy().astype(np.float64)[idx] - lq_o) <= lq_bound(lq_o, picked)).all()
+    check_own_sum(lq_g.cpu().numpy().astype(np.float64), cp_g.cpu().numpy().astype(np.float64), spins_g.cpu().numpy())
+    lq_tf, cp_tf = model.log_prob(spins_g, want_cond_p=True)
+    assert (cp_tf - cp_g).abs().max().item() <= 2e-4
+    again = model.sample(dev(u), want_cond_p=True)
+    assert all(torch.equal(x, y) for x, y in zip((spins_g, lq_g, cp_g), again))      # bit-reproducible
+    print(f"tcgen05 streaming sampler {case} B={B}: {len(idx)} samples against the oracle, near-tie sites {int(tie.sum())}, flips {int(mism.sum())}")
+    model.close()
+
+
 def test_chain_sampler_refuses_uncovered_shapes(monkeypatch):
     w = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2)       # d = 64
     model, weights, posemb, rp, col = build(w, 8)
