@@ -47,7 +47,7 @@ def parse():
 def sampler_source_hash():
     """sha256 over the sources of the fv_sample kernels: a committed ncu figure is only quoted while they are unchanged."""
     h = hashlib.sha256()
-    for f in ("fv_chain.cu", "fv_decode.cu", "fv_ring.cuh", "fv_device.cuh", "fv_umma.cuh"):
+    for f in ("fv_chain.cu", "fv_decode.cu", "fv_decode_tc.cu", "fv_ring.cuh", "fv_device.cuh", "fv_umma.cuh"):
         h.update(open(os.path.join(ROOT, "paper_2606_22984_b200", "csrc", f), "rb").read())
     return h.hexdigest()[:16]
 
@@ -60,7 +60,7 @@ def ncu_traffic(workload, batch, kind="ring"):
     if not os.path.exists(path):
         return None, "no profiles/sampler_traffic.csv"
     rows = [r for r in csv.DictReader(l for l in open(path) if not l.startswith("#"))
-            if r["workload"].split("_")[0] == workload and int(r["batch"]) == batch and ("chain" in r["kernel"]) == (kind == "chain")]
+            if r["workload"] == workload and int(r["batch"]) == batch and r["sampler"] == kind]
     if not rows:
         return None, f"no ncu capture of {workload} at batch {batch} in profiles/sampler_traffic.csv"
     r = rows[-1]
@@ -358,8 +358,9 @@ def run_ours(args):
             "us_per_site_step": 1e3 * t_sample / N,
             "F_q": {"mean": Fq_mean, "std": Fq_std, "per_spin": Fq_mean / N,
                     "rank0_kernel": [float(F_val[0]), float(F_val[1])]},
-            "roofline": {"kernel": ("fv_chain_kernel (fv_sample: layer-pipelined clusters, weights resident in TMEM / shared memory)"
-                                    if sampler_kind == "chain" else "fv_decode_kernel (fv_sample: persistent KV-ring sampler)"),
+            "roofline": {"kernel": {"chain": "fv_chain_kernel (fv_sample: layer-pipelined clusters, weights resident in TMEM / shared memory)",
+                                    "ring-tc": "fv_decode_tc_kernel (fv_sample: persistent KV-ring sampler, projections on tcgen05)",
+                                    "ring": "fv_decode_kernel (fv_sample: persistent KV-ring sampler, projections on mma.sync)"}[sampler_kind],
                          "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "achieved_is": "ALGORITHMIC KV bytes (rows the mask names: read + append) / kernel duration; L2 hits "
                                         "between consecutive steps make the DRAM bytes smaller, see dram_*",
