@@ -186,8 +186,16 @@ const char* fv_sampler_kind(const fv_model* m, int32_t B);
  * Synchronises on the recorded events (i.e. on the work they bracket). */
 int fv_profile(int32_t enable, double* ms, int64_t* launches);
 
-/* Bytes of device memory the model's KV pool occupies (0 for NULL). */
+/* Bytes of device memory fv_sample's KV pool occupies (0 for NULL). */
 int64_t fv_kv_bytes(const fv_model* m);
+
+/* Band-only fast path (Eq. S1: M_ij = 0 iff i - j <= W).  When every mask row t is
+ * the single run max(0, t-W)..t and 2(W+1) <= N, fv_create_model gives fv_sample a ring-buffer KV window of W+1 rows per
+ * (sample, layer) instead of N rows -- position p lives in row p mod (W+1), results are bit-identical to the N-row pool --
+ * and fv_log_prob allocates its own N-row pool at its first call (cudaMalloc: that one call synchronises the device).
+ * Returns W+1 for such a model, 0 otherwise (and for NULL).  FLASHVAN_KV=dense in the environment at fv_create_model
+ * time keeps the N-row pool (A/B measurements). */
+int32_t fv_kv_window(const fv_model* m);
 
 /* Number of kernel launches the library has enqueued since load (for bench.py gpu_launches). */
 int64_t fv_launch_count(void);

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.so")
 
 SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
-           "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_launch_count",
+           "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_kv_window", "fv_launch_count",
            "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps", "fv_profile", "fv_sampler_kind", "fv_tokens_to_spins"]
 
 
@@ -54,6 +54,8 @@ def lib() -> ctypes.CDLL:
         L.fv_n_weights.restype = i64
         L.fv_kv_bytes.argtypes = [vp]
         L.fv_kv_bytes.restype = i64
+        L.fv_kv_window.argtypes = [vp]
+        L.fv_kv_window.restype = ctypes.c_int32
         L.fv_launch_count.restype = i64
         L.fv_last_error.restype = ctypes.c_char_p
         L.fv_lmc_sweeps.argtypes = [i32, i32, i32, vp, vp, vp, vp, ctypes.c_float, vp, vp, vp]
@@ -133,6 +135,11 @@ class Model:
     @property
     def kv_bytes(self) -> int:
         return int(lib().fv_kv_bytes(self._h))
+
+    @property
+    def kv_window(self) -> int:
+        """Rows of fv_sample's ring-buffer KV window for a band mask (Eq. S1), 0 for any other mask."""
+        return int(lib().fv_kv_window(self._h))
 
     def sample(self, uniforms: torch.Tensor, want_cond_p: bool = False, out=None):
         """fv_sample: uniforms [B,N] f32 cuda -> (spins int8 [B,N], logq f32 [B], cond_p or None)."""

@@ -22,6 +22,8 @@ struct fv_model {
     int n_sms = 0;
     int device = 0;
     double mean_nnz = 0.0;       // mask entries per row
+    int window = 0;              // > 0: band mask, fv_sample's pool is a ring-buffer window of this many rows per stream
+    size_t kv_full_bytes = 0;    // fv_log_prob's pool [max_batch][n_layers][N][2d] (window mode: allocated at its first call)
 };
 
 namespace {
@@ -166,6 +168,7 @@ const char* fv_last_error(void) { return g_err.c_str(); }
 int64_t fv_launch_count(void) { return g_launches.load(); }
 int64_t fv_n_weights(const fv_config* cfg) { return shape_ok(cfg) ? n_weights_of(cfg) : -1; }
 int64_t fv_kv_bytes(const fv_model* m) { return m ? (int64_t)m->kv_bytes : 0; }
+int32_t fv_kv_window(const fv_model* m) { return m ? m->window : 0; }
 
 int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weights, const int32_t* mask_rowptr,
                     const int32_t* mask_col, const float* posemb, void* stream, fv_model** out) {
@@ -272,6 +275,17 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     const size_t o_col = A.put(mask_col, sizeof(int32_t) * (size_t)mask_rowptr[N]);
     // KV ring copy plan (fv_decode.cu): chunks of CH rows of A(t) \ {t}, runs of consecutive positions
     const int CH = fv_ring_ch(d);
+    // Band mask (Eq. S1: M_ij = 0 iff i - j <= W): every row is the ONE run max(0, t-W)..t.  fv_sample then keeps
+    // only a ring-buffer window of W+1 rows per (sample, layer): position p lives in row p % (W+1); the row step t appends
+    // overwrites position t-W-1, which no later step attends.  FLASHVAN_KV=dense keeps the N-row pool (A/B measurements).
+    int band_w = 0;
+    for (int t = 0; t < N; ++t) band_w = std::max(band_w, t - mask_col[mask_rowptr[t]]);
+    bool band = band_w >= 1 && 2 * (band_w + 1) <= N;
+    for (int t = 0; t < N && band; ++t)
+        band = mask_col[mask_rowptr[t]] == std::max(0, t - band_w) && mask_rowptr[t + 1] - mask_rowptr[t] == t - mask_col[mask_rowptr[t]] + 1;
+    if (const char* kvm = std::getenv("FLASHVAN_KV"); kvm && std::strcmp(kvm, "dense") == 0) band = false;
+    const int kv_rows = band ? band_w + 1 : N;
+    m->window = band ? kv_rows : 0;
     std::vector<int32_t> chunk_ptr(N + 1, 0), chunk_run_ptr(1, 0);
     std::vector<int2> runs;
     for (int t = 0; t < N; ++t) {
@@ -280,8 +294,9 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
             const int rows = std::min(CH, nn - c0);
             for (int i = 0; i < rows;) {
                 int j = i + 1;
-                while (j < rows && mask_col[e0 + c0 + j] == mask_col[e0 + c0 + j - 1] + 1) ++j;
-                runs.push_back(make_int2(mask_col[e0 + c0 + i], (i << 16) | (j - i)));
+                while (j < rows && mask_col[e0 + c0 + j] == mask_col[e0 + c0 + j - 1] + 1 &&
+                       mask_col[e0 + c0 + j] % kv_rows != 0) ++j;          // a run ends where the window wraps
+                runs.push_back(make_int2(mask_col[e0 + c0 + i] % kv_rows, (i << 16) | (j - i)));
                 i = j;
             }
             chunk_run_ptr.push_back((int32_t)runs.size());
@@ -322,7 +337,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     m->arena_bytes = A.host.size();
     e = cudaMalloc(&m->arena, m->arena_bytes);
     if (e != cudaSuccess) { delete m; return cuda_fail(e, "cudaMalloc(parameters)"); }
-    m->kv_bytes = (size_t)cfg->max_batch * NL * N * 2 * d * sizeof(__nv_bfloat16);
+    m->kv_full_bytes = (size_t)cfg->max_batch * NL * N * 2 * d * sizeof(__nv_bfloat16);
+    m->kv_bytes = (size_t)cfg->max_batch * NL * kv_rows * 2 * d * sizeof(__nv_bfloat16);
     void* kv = nullptr;
     e = cudaMalloc(&kv, m->kv_bytes);
     if (e != cudaSuccess) { cudaFree(m->arena); delete m; return cuda_fail(e, "cudaMalloc(KV pool)"); }
@@ -358,7 +374,9 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.att_ukeys = (const int32_t*)(base + o_uk);
     D.att_mask = (const uint16_t*)(base + o_am);
     D.att_nblk = n_blk;
-    D.kv = (__nv_bfloat16*)kv;
+    D.kv_s = (__nv_bfloat16*)kv;
+    D.kv_rows = kv_rows;
+    D.kv = band ? nullptr : (__nv_bfloat16*)kv;       // window mode: fv_log_prob allocates its N-row pool at its first call
     D.lp_h = (float*)m->ws;
     D.lp_q = m->ws ? (float*)m->ws + (size_t)cfg->max_batch * N * d : nullptr;
     for (int l = 0; l < NL; ++l) {
@@ -388,7 +406,8 @@ void fv_destroy_model(fv_model* m) {
     cudaGetDevice(&cur);
     if (cur != m->device) cudaSetDevice(m->device);      // free on the model's own device, then restore
     cudaDeviceSynchronize();
-    cudaFree(m->dev.kv);
+    if (m->dev.kv != m->dev.kv_s) cudaFree(m->dev.kv);
+    cudaFree(m->dev.kv_s);
     cudaFree(m->ws);
     cudaFree(m->arena);
     if (cur >= 0 && cur != m->device) cudaSetDevice(cur);
@@ -502,6 +521,12 @@ int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float*
     if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
     if (B <= 0 || B > m->cfg.max_batch) return fail(FV_ERR_BAD_ARG, "B must be in [1, max_batch]");
     if (int rc = wrong_device(m)) return rc;
+    if (!m->dev.kv) {                                              // window mode: the teacher-forced pass needs all N rows
+        void* kv = nullptr;
+        cudaError_t ea = cudaMalloc(&kv, m->kv_full_bytes);
+        if (ea != cudaSuccess) return cuda_fail(ea, "cudaMalloc(fv_log_prob KV pool)");
+        m->dev.kv = (__nv_bfloat16*)kv;
+    }
     const char* force = std::getenv("FLASHVAN_LOGPROB");          // "chunked": the persistent teacher-forcing kernel
     if (m->dev.vocab > 2) force = nullptr;                         // (one spin per token only)
     if (!(force && std::strcmp(force, "chunked") == 0)) {

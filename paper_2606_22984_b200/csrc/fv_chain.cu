@@ -223,7 +223,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                     const int need = (t - 1) * MBc + mb + 1;
                     while (ld_acquire_s32(sh_app) < need) __nanosleep(32);
                 }
-                const unsigned char* src_l = reinterpret_cast<const unsigned char*>(m.kv + ((size_t)b_first * NL + l) * N * (2 * D));
+                const unsigned char* src_l = reinterpret_cast<const unsigned char*>(m.kv_s + ((size_t)b_first * NL + l) * m.kv_rows * (2 * D));
                 for (int i0 = 0; i0 < total;) {
                     const int i = i0 + lane;
                     const uint32_t sq = seq + (uint32_t)i;
@@ -236,7 +236,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                         const int r = k * GR + (rem - c * nk);
                         const int rows = min(CH, nn - c * CH);
                         mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * ROW_BYTES);
-                        const unsigned char* src = src_l + (size_t)r * NL * N * ROW_BYTES;
+                        const unsigned char* src = src_l + (size_t)r * NL * m.kv_rows * ROW_BYTES;
                         unsigned char* dst = ring + (size_t)slot * CHUNK_BYTES;
                         const int j1 = cur.cptr[c + 1];
                         for (int j = cur.cptr[c]; j < j1; ++j) {
@@ -363,7 +363,7 @@ fv_chain_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ Ch
                 const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
                 if (r >= n_own) continue;
                 const uint4 v = *reinterpret_cast<const uint4*>(sh_kv + r * KVS + ch * 8);
-                __nv_bfloat16* dst = m.kv + (((size_t)(b_first + r) * NL + l) * N + t) * (2 * D) + ch * 8;
+                __nv_bfloat16* dst = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + t % m.kv_rows) * (2 * D) + ch * 8;
                 *reinterpret_cast<uint4*>(dst) = v;
             }
             asm volatile("fence.proxy.async.global;\n" ::: "memory");   // the producer reads these rows by cp.async.bulk

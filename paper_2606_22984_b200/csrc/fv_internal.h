@@ -56,7 +56,12 @@ struct FvModelDev {
     const int32_t* chunk_ptr;      // [N+1]  chunks before step t
     const int32_t* chunk_run_ptr;  // [n_chunks+1]
     const int2* runs;
-    __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16)
+    __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16); fv_log_prob's pool
+    // fv_sample's pool: the same array, or -- when every mask row is one run t-W..t (the band of Eq. S1) --
+    // a ring-buffer window [max_batch][n_layers][kv_rows = W+1][2d] in which position p lives in row p % kv_rows
+    // (the copy plan's run.x is then that physical row, runs cut at the wrap)
+    __nv_bfloat16* kv_s;
+    int32_t kv_rows;        // rows per (sample, layer) stream of kv_s: N, or W+1 in window mode
     // fv_logprob.cu block attention plan: per block of 32 queries the padded union of key positions and,
     // per 16-key step and query, a 16-bit allow mask
     const int32_t* att_blk_uptr;   // [att_nblk + 1] offsets into att_ukeys (multiples of 16)
