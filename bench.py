@@ -192,10 +192,12 @@ def spawn_ranks(args):
     raise SystemExit(subprocess.call(cmd, env=env))
 
 
-def time_other_config(fv, torch, name, w, B, steps=3, seed_u=None):
+def time_other_config(fv, torch, name, w, B, steps=3, seed_u=None, mask=None):
     """Short timing of fv_sample / fv_log_prob on another BASELINE config (the headline's model is closed by
     then): CUDA events, one warm-up pass, `steps` timed passes."""
     inp = W.make_all(w, batch=B) if seed_u is None else W.make_all(w, batch=B, u_seed=seed_u)
+    if mask is not None:
+        inp["mask_rowptr"], inp["mask_col"] = mask
     model = fv.create_model(w, inp["weights"], inp["mask_rowptr"], inp["mask_col"], inp["posemb"], B)
     u = torch.from_numpy(np.ascontiguousarray(inp["uniforms"])).cuda()
     spins = torch.empty((B, w.n_sites), dtype=torch.int8, device="cuda")
@@ -212,6 +214,7 @@ def time_other_config(fv, torch, name, w, B, steps=3, seed_u=None):
     ts = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(steps)) / steps
     tl = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(steps)) / steps
     chain_gap = float((logq - lq2).abs().max().item())
+    kv_window, kv_pool = model.kv_window, model.kv_bytes
     model.close()
     rd, wr = algorithmic_kv_bytes_per_sample(w, inp["mask_rowptr"])
     peak, _, _ = load_peaks()
@@ -219,6 +222,8 @@ def time_other_config(fv, torch, name, w, B, steps=3, seed_u=None):
     out = {"workload": name, "batch": B, "fv_sample_ms": ts, "fv_log_prob_ms": tl, "samples_per_s": B / ((ts + tl) * 1e-3),
            "us_per_site_step": 1e3 * ts / w.n_sites, "algorithmic_kv_frac_of_hbm_peak": (rd + wr) * B / (ts * 1e-3) / 1e9 / peak,
            "max_abs_logq_sample_vs_log_prob": chain_gap}
+    if kv_window:
+        out["kv_window_rows"], out["kv_pool_bytes"] = kv_window, kv_pool
     out["bound"] = "latency (KV traffic of a site step is %.1f us at the HBM peak)" % kv_us if kv_us < 10.0 else "hbm"
     return out
 
@@ -390,6 +395,13 @@ def run_ours(args):
             import dataclasses
             others.append(time_other_config(fv, torch, "cfg5 with W_O (has_wo = 1, reading A8)",
                                             dataclasses.replace(w, has_wo=1), B))
+            # the same model at four times BASELINE's batch (28 instead of 7 samples per SM share one weight stream), and
+            # the band-only fast path: the open-boundary 64 x 64 lattice's exact mask, previous L spins
+            # (PAPER.md:549), whose KV lives in a ring-buffer window of W + 1 rows -- which is what lets the batch grow
+            others.append(time_other_config(fv, torch, "cfg5 at B = 4096 (28 samples per SM)", w, 4 * B))
+            band = W.band_mask_csr(w.n_sites, w.L)
+            others.append(time_other_config(fv, torch, "cfg5 model, pure band W = 64 (Eq. S1), B = 1024", w, B, mask=band))
+            others.append(time_other_config(fv, torch, "cfg5 model, pure band W = 64 (Eq. S1), B = 4096", w, 4 * B, mask=band))
             out["other_configs"] = others
         if world == 1 and not args.no_cpu_baseline:
             from oracle import oracle as O
