@@ -100,6 +100,24 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p,
                 void* stream);
 
+/* fv_log_prob for callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same kernels and the same results, bit for bit, but the call's workspace -- the residual stream h
+ * and the queries q (fp32 [B*N, d_model] each) and the layer-major K|V rows (bf16 [B][n_layers][N][2 d_model]) -- lives
+ * in ONE file-scope `static __device__` array of FV_STATIC_SCRATCH_BYTES inside the library instead of the model's
+ * own buffers.  Every GPU that loads the library holds that array until the process exits.  The call itself makes no
+ * cudaMalloc / cudaFree / allocating library call (keep fv_profile off: its events are created on demand); the first
+ * call on a device looks the array's address up once (cudaGetSymbolAddress).
+ *   Limit: B * N * d_model * (8 + 4 * n_layers) bytes (+ alignment) <= FV_STATIC_SCRATCH_BYTES, i.e. 16 384 rows
+ *   (B * N) for a 6-layer d_model = 128 model; larger calls return FV_ERR_BAD_ARG and fv_last_error() names the
+ *   bytes needed.  Shapes the layer-major path does not cover (has_wo, d_model = 256) return FV_ERR_BAD_SHAPE.
+ *   The array is shared by every model and every call on the device and keeps the previous call's contents; nothing
+ *   in it needs clearing (each call writes every row before reading it), but two calls that overlap on the GPU
+ *   (different streams, or two host threads) race on it: order them on one stream.  The model's KV pool is untouched.
+ * Arguments, outputs and error codes otherwise as fv_log_prob. */
+#define FV_STATIC_SCRATCH_BYTES (64u << 20)
+int fv_log_prob_static(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p,
+                       void* stream);
+
 /* Eq. 8: E_b = - sum over listed bonds J_ij s_i s_j, every bond listed once.
  *   rowptr [device] N+1, col [device], val [device] fp32: CSR of the bonds (any triangle).
  *   integer_couplings != 0: every val is an integer; the sum is taken in int32 and is exact.

@@ -15,7 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("FLASHVAN_LIB") or os.path.join(_HERE, "libflashvan.so")
 
-SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_energy_csr", "fv_energy_dense",
+SYMBOLS = ["fv_create_model", "fv_sample", "fv_log_prob", "fv_log_prob_static", "fv_energy_csr", "fv_energy_dense",
            "fv_free_energy", "fv_destroy_model", "fv_n_weights", "fv_kv_bytes", "fv_kv_window", "fv_launch_count",
            "fv_last_error", "fv_markov_mask", "fv_overlap", "fv_lmc_sweeps", "fv_profile", "fv_sampler_kind", "fv_tokens_to_spins"]
 
@@ -45,6 +45,7 @@ def lib() -> ctypes.CDLL:
         L.fv_create_model.argtypes = [ctypes.POINTER(FvConfig), vp, i64, vp, vp, vp, vp, ctypes.POINTER(vp)]
         L.fv_sample.argtypes = [vp, i32, vp, vp, vp, vp, vp]
         L.fv_log_prob.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.fv_log_prob_static.argtypes = [vp, i32, vp, vp, vp, vp]
         L.fv_energy_csr.argtypes = [i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.fv_energy_dense.argtypes = [i32, i32, vp, vp, vp, vp]
         L.fv_free_energy.argtypes = [i32, vp, vp, ctypes.c_double, vp, vp]
@@ -167,6 +168,20 @@ class Model:
         cp = torch.empty((B, N), dtype=torch.float32, device=s.device) if want_cond_p else None
         _check(lib().fv_log_prob(self._h, B, s.data_ptr(), logq.data_ptr(),
                                  cp.data_ptr() if cp is not None else None, _stream()), "fv_log_prob")
+        return logq, cp
+
+    def log_prob_static(self, spins: torch.Tensor, logq: torch.Tensor, cond_p: torch.Tensor = None):
+        """fv_log_prob_static: fv_log_prob with its workspace in the library's static device array -- no allocation,
+        here or in the library (the caller passes the outputs: logq f32 [B], cond_p f32 [B,N] or None).  Calls that
+        overlap on the GPU race on that array; B * N is limited (flashvan.h: FV_STATIC_SCRATCH_BYTES)."""
+        s = _dev(spins, torch.int8)
+        B, N = s.shape
+        if N != self.cfg.n_sites or s.device != self.device:
+            raise FlashVanError(f"spins must be [B, n_sites] on {self.device}")
+        logq = _out(logq, torch.float32, (B,), s)
+        cp = _out(cond_p, torch.float32, (B, N), s) if cond_p is not None else None
+        _check(lib().fv_log_prob_static(self._h, B, s.data_ptr(), logq.data_ptr(),
+                                        cp.data_ptr() if cp is not None else None, _stream()), "fv_log_prob_static")
         return logq, cp
 
     def sampler_kind(self, B: int) -> str:

@@ -553,6 +553,28 @@ int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float*
     return FV_OK;
 }
 
+static_assert(FV_LP_STATIC_BYTES == FV_STATIC_SCRATCH_BYTES, "flashvan.h and fv_internal.h disagree on the static scratch size");
+
+int fv_log_prob_static(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p, void* stream) {
+    if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
+    if (B <= 0) return fail(FV_ERR_BAD_ARG, "B must be positive");
+    if (int rc = wrong_device(m)) return rc;
+    if (m->cfg.has_wo || m->cfg.d_model > 128)
+        return fail(FV_ERR_BAD_SHAPE, "fv_log_prob_static: only the layer-major path (d_model <= 128, no W_O)");
+    const size_t need = fv_logprob_static_need(m->dev, m->cfg.d_model, B);
+    if (need > FV_LP_STATIC_BYTES)
+        return fail(FV_ERR_BAD_ARG, "fv_log_prob_static: B * N = " + std::to_string((long long)B * m->cfg.n_sites) + " rows need " +
+                                        std::to_string(need) + " bytes of workspace, the static array holds " +
+                                        std::to_string(FV_LP_STATIC_BYTES) + " (use fv_log_prob)");
+    int n_launch = 0;
+    cudaError_t e = fv_launch_logprob_tc_static(m->dev, m->cfg.d_model, m->cfg.d_model / m->cfg.n_heads, B, spins, logq, cond_p,
+                                                m->n_sms, &n_launch, (cudaStream_t)stream);
+    if (e == cudaErrorNotSupported) { (void)cudaGetLastError(); return fail(FV_ERR_BAD_SHAPE, "fv_log_prob_static: shape not covered by the layer-major path"); }
+    if (e != cudaSuccess) return cuda_fail(e, "fv_log_prob_static launch");
+    g_launches += n_launch;
+    return FV_OK;
+}
+
 int fv_energy_csr(int32_t B, int32_t N, const int8_t* spins, const int32_t* rowptr, const int32_t* col,
                   const float* val, int32_t integer_couplings, float* E, void* stream) {
     if (!spins || !rowptr || !col || !val || !E) return fail(FV_ERR_BAD_ARG, "null argument");

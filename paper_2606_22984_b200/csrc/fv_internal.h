@@ -122,6 +122,11 @@ bool fv_chain_supported(const FvModelDev& m, int d_model, int d_head, int B);
 cudaError_t fv_launch_chain(const FvModelDev& m, int d_model, int d_head, const FvForwardArgs& a, cudaStream_t s);
 cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
                                  float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s);
+// fv_log_prob_static (flashvan.h): workspace of one call in a file-scope __device__ array of this size
+constexpr size_t FV_LP_STATIC_BYTES = (size_t)64 << 20;
+size_t fv_logprob_static_need(const FvModelDev& m, int d_model, int B);
+cudaError_t fv_launch_logprob_tc_static(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
+                                        float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s);
 void fv_pack_sw128(const float* W, int rows, int K, int ld, int KP, uint16_t* dst);
 cudaError_t fv_launch_energy_csr(int B, int N, const int8_t* spins, const int32_t* rowptr,
                                  const int32_t* col, const float* val, int integer, float* E,

@@ -972,6 +972,50 @@ cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, i
     }
 }
 
+// ---- fv_log_prob_static: the same launches with the workspace in a file-scope array ---------------------------
+// For callers that cannot allocate (CUDA graph capture, serving loops): h, q and the layer-major K|V rows of ONE call
+// live in this array instead of the model's cudaMalloc'ed workspace and pool.  Every GPU that loads the library holds
+// the FV_LP_STATIC_BYTES until the process exits.  In host code the array's name is only a stand-in for the symbol,
+// not a device address: the address comes from cudaGetSymbolAddress, once per device, with that device current.
+// Nothing in it has to start at zero -- lp_qkv_kernel writes every h / q / K|V row of the B samples (padding keys of
+// the attention plan are position 0, a written row) before any kernel reads it -- so the contents the previous call
+// left behind are simply overwritten; two calls that overlap on the GPU (different streams) race on it.
+static __device__ __align__(256) unsigned char g_lp_static[FV_LP_STATIC_BYTES];
+
+size_t fv_logprob_static_need(const FvModelDev& m, int d_model, int B) {
+    const size_t rows = (size_t)B * m.n_sites;
+    const size_t act = (rows * d_model * sizeof(float) + 255) / 256 * 256;                 // h, then q
+    return 2 * act + rows * m.n_layers * 2 * d_model * sizeof(__nv_bfloat16);              // then [B][n_l][N][2d] K|V
+}
+
+cudaError_t fv_launch_logprob_tc_static(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins,
+                                        float* logq, float* cond_p, int n_sms, int* n_launches, cudaStream_t s) {
+    if (fv_logprob_static_need(m, d_model, B) > FV_LP_STATIC_BYTES) return cudaErrorInvalidValue;
+    static std::mutex mu;
+    static std::map<int, unsigned char*> base_of;            // device -> address of g_lp_static there
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    unsigned char* base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        auto it = base_of.find(dev);
+        if (it == base_of.end()) {
+            e = cudaGetSymbolAddress((void**)&base, g_lp_static);
+            if (e != cudaSuccess) return e;
+            base_of[dev] = base;
+        } else {
+            base = it->second;
+        }
+    }
+    const size_t act = ((size_t)B * m.n_sites * d_model * sizeof(float) + 255) / 256 * 256;
+    FvModelDev ms = m;                                       // same parameters, plans and images; other workspace
+    ms.lp_h = reinterpret_cast<float*>(base);
+    ms.lp_q = reinterpret_cast<float*>(base + act);
+    ms.kv = reinterpret_cast<__nv_bfloat16*>(base + 2 * act);
+    return fv_launch_logprob_tc(ms, d_model, d_head, B, spins, logq, cond_p, n_sms, n_launches, s);
+}
+
 // Host side of the images the kernels above copy verbatim into shared memory: W[rows, K] (row
 // stride ld, fp32) -> bf16, K-major, SWIZZLE_128B, K padded to KP: K-block kb of 64 columns is a
 // [rows x 128 B] slab, 8-row groups 1024 B apart, 16-byte chunk c of row r at chunk c ^ (r & 7).
