@@ -22,6 +22,9 @@ namespace {
 using namespace fvring;
 
 constexpr int NTHREADS = NWC * 32 + 32;       // compute warps + the producer warp
+#ifndef FV_DEC_WG
+#define FV_DEC_WG 2
+#endif
 constexpr int GEMM_MAXL = 8;                  // 128-bit weight loads in flight per lane when the weights come by LDG (d = 256)
 
 // CL = the CTA is one half of a 2-CTA cluster that splits the FFN (see the kernel header).
@@ -60,7 +63,12 @@ struct DecGeo {
     static constexpr size_t bar_bytes = 1024 + 2 * (TAB_C * 4 + TAB_R * 8);   // mbarriers (2 x 60 + 2), counters, plans
     static constexpr int NSLOT_RAW = (int)((SMEM_MAX - fixed - bar_bytes) / CHUNK_BYTES);
     static constexpr int NSLOT_CAP = 60;
-    static constexpr int NSLOT = NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW;
+    // Weight chunks travel in groups of WG consecutive chunks = ONE bulk copy of WG * CHUNK_BYTES into WG adjacent slots
+    // (the TMA unit costs ~30 ns per copy + 4.4 ns per KB: 8 KB copies feed an SM with 124 GB/s, 16 KB with 163 GB/s, and
+    // the stream is what the compute warps wait for).  Groups never wrap: NSLOT is a multiple of WG and every section of
+    // the chunk sequence (a weight matrix, the KV chunks of a layer-step padded with empty chunks) is one too.
+    static constexpr int WG = (!CL && D == 128) ? FV_DEC_WG : 1;
+    static constexpr int NSLOT = (NSLOT_RAW > NSLOT_CAP ? NSLOT_CAP : NSLOT_RAW) / WG * WG;
     static constexpr size_t total = fixed + bar_bytes + (size_t)NSLOT * CHUNK_BYTES;
     // GEMM weights stream through the same ring (D <= 128): a chunk is CHUNK_BYTES of the packed
     // image = TPCH 16x16 tiles = whole m-tiles (K = D) or one K-part of an m-tile (K = 4D).
@@ -74,11 +82,23 @@ struct DecGeo {
 };
 
 
+// Weight chunk sq of a group of WG chunks that arrived with one bulk copy: the bytes complete on the full barrier of
+// the group's FIRST slot (sections start at multiples of WG, so sq % WG is the chunk's place in its group).
+template <int NSLOT, int CHUNK_BYTES, int WG>
+__device__ __forceinline__ unsigned char* ring_acquire_w(const RingCtx& rc, uint32_t sq, uint32_t& slot) {
+    if constexpr (WG == 1) return ring_acquire<NSLOT, CHUNK_BYTES>(rc, sq, slot);
+    slot = sq % NSLOT;
+    const uint32_t s0 = sq - sq % WG;
+    while ((int)((uint32_t)ld_acquire_s32(rc.issued) - sq) <= 0) __nanosleep(20);
+    mbar_wait(rc.bar_full + s0 % NSLOT, (s0 / NSLOT) & 1u);
+    return rc.ring + (size_t)slot * CHUNK_BYTES;
+}
+
 // GEMM over one tile of 8*NT rows with the weights taken from ring chunks (same contract as
 // gemm_rows).  Chunk j of a matrix holds TPCH consecutive 16x16 tiles of its packed image:
 // MPC whole m-tiles when K fits a chunk, else K-part (j % KSP) of m-tile j / KSP.  Warp w
 // consumes chunks w, w + NWC, ... (ring order), A fragments by conflict-free 128-bit LDS.
-template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, class Epi>
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, class Epi>
 __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32_t seq0, const __nv_bfloat16* act,
                                           int as, int warp, int lane, Epi epi) {
     constexpr bool SPLITK = KT_TOTAL > TPCH;
@@ -88,7 +108,7 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
     const int g = lane >> 2, c = lane & 3;
     for (int j = warp; j < nchunks; j += NWC) {
         uint32_t slot;
-        const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)j, slot)) + lane;
+        const uint4* wsm = reinterpret_cast<const uint4*>(ring_acquire_w<NSLOT, CHUNK_BYTES, WG>(rc, seq0 + (uint32_t)j, slot)) + lane;
         const int ks = SPLITK ? j - (j / KSP) * KSP : 0;
         const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
         // k outer, m-tiles inner: the activation fragments of a k-step are read once and feed MPC (K = D)
@@ -137,7 +157,7 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
 // W2 GEMM (K = 4D > one chunk) with all KSP K-parts of an m-tile consumed by the SAME warp, one after the
 // other (ring order), into one accumulator: no partial-sum buffer and no separate reduction phase --
 // epi(mt, acc) applies bias and residual directly.
-template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, class Epi>
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, class Epi>
 __device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles, uint32_t seq0, const __nv_bfloat16* act,
                                                  int as, int warp, int lane, Epi epi) {
     static_assert(KT_TOTAL % TPCH == 0 && KT_TOTAL > TPCH, "K must span several chunks");
@@ -153,7 +173,7 @@ __device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles
         for (int ks = 0; ks < KSP; ++ks) {
             uint32_t slot;
             const uint4* wsm = reinterpret_cast<const uint4*>(
-                ring_acquire<NSLOT, CHUNK_BYTES>(rc, seq0 + (uint32_t)(mt * KSP + ks), slot)) + lane;
+                ring_acquire_w<NSLOT, CHUNK_BYTES, WG>(rc, seq0 + (uint32_t)(mt * KSP + ks), slot)) + lane;
             const __nv_bfloat16* ab = act + g * as + ks * KT * 16 + 2 * c;
 #pragma unroll
             for (int kt = 0; kt < KT; ++kt) {
@@ -257,6 +277,32 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         };
         // one weight matrix = n consecutive CHUNK_BYTES pieces of its packed image, one copy each
         auto issue_weights = [&](const uint4* w, int n, int first = 0, int stride = 1) {
+            if constexpr (DG::WG > 1) {                 // groups of WG chunks: one copy, bytes counted on the first slot
+                constexpr int WG = DG::WG, GB = WG * DG::CHUNK_BYTES;
+                const unsigned char* srcg = reinterpret_cast<const unsigned char*>(w);
+                const int ng = n / WG;
+                for (int g0 = 0; g0 < ng;) {
+                    const int gi = g0 + lane;
+                    const uint32_t sq = seq + (uint32_t)(gi * WG);
+                    const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                    bool ok = lane < VW / WG && gi < ng;
+#pragma unroll
+                    for (int k = 0; k < WG; ++k) ok = ok && mbar_test(bar_empty + slot + k, par ^ 1u);
+                    const unsigned int bm = __ballot_sync(0xffffffffu, ok);
+                    const int npre = bm == 0xffffffffu ? 32 : __ffs(~bm) - 1;
+                    if (lane < npre) {
+                        mbar_arrive_expect_tx(bar_full + slot, (uint32_t)GB);
+#pragma unroll
+                        for (int k = 1; k < WG; ++k) mbar_arrive(bar_full + slot + k);
+                        bulk_g2s(ring + (size_t)slot * DG::CHUNK_BYTES, srcg + (size_t)gi * GB, (uint32_t)GB, bar_full + slot);
+                    }
+                    __syncwarp();
+                    g0 += npre;
+                    if (lane == 0 && npre) st_release_s32(sh_issued, (int)(seq + (uint32_t)(g0 * WG)));
+                }
+                seq += (uint32_t)n;
+                return;
+            }
             const unsigned char* src = reinterpret_cast<const unsigned char*>(w) + (size_t)first * DG::CHUNK_BYTES;
             for (int i0 = 0; i0 < n;) {
                 const int i = i0 + lane;
@@ -347,6 +393,20 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         if (lane == 0 && npre) st_release_s32(sh_issued, (int)(seq + (uint32_t)i0));
                     }
                     seq += (uint32_t)total;
+                    if constexpr (DG::WG > 1) {           // empty chunks up to the next multiple of WG: armed and released here
+                        const int pad = (DG::WG - total % DG::WG) % DG::WG;
+                        if (lane == 0)
+                            for (int k = 0; k < pad; ++k) {
+                                const uint32_t sq = seq + (uint32_t)k;
+                                const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
+                                while (!mbar_test(bar_empty + slot, par ^ 1u)) {}
+                                mbar_arrive(bar_full + slot);
+                                mbar_arrive(bar_empty + slot);
+                            }
+                        __syncwarp();
+                        seq += (uint32_t)pad;
+                        if (lane == 0 && pad) st_release_s32(sh_issued, (int)seq);
+                    }
                     if (DG::WRING) {
                         if (m.has_wo) issue_weights(L.wo, DG::NO);
                         if (CL) {     // my half of the hidden layer: rows of W1, K-half of every m-tile of W2
@@ -416,7 +476,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                     };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NQ;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
@@ -501,6 +561,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     }
                 }
                 seq_base += (uint32_t)(n_own * nch);
+                if constexpr (DG::WG > 1) seq_base += (uint32_t)((DG::WG - (n_own * nch) % DG::WG) % DG::WG);
                 cbar();
                 if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 if (NSPLIT > 1) {                       // combine the split partials, fixed order
@@ -538,7 +599,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NO;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
@@ -575,13 +636,15 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
 #pragma unroll
                             for (int nt = 0; nt < NT2; ++nt) {
                                 __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS2 + f;
-                                o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
-                                o[FS2] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
-                                o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
-                                o[FS2 + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
+                                // exact-erf GELU by the one-ex2 erfc form (fv_device.cuh; erff cost a tenth of the kernel's issue slots)
+                                const uint32_t g0 = gelu_erfc_x2(acc[nt][0] + b0, acc[nt][1] + b0);
+                                const uint32_t g1 = gelu_erfc_x2(acc[nt][2] + b1, acc[nt][3] + b1);
+                                uint16_t* ou = reinterpret_cast<uint16_t*>(o);
+                                ou[0] = (uint16_t)g0; ou[FS2] = (uint16_t)(g0 >> 16);
+                                ou[8] = (uint16_t)g1; ou[FS2 + 8] = (uint16_t)(g1 >> 16);
                             }
                         };
-                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
                         seq_base += DG::N1 / 2;
                     }
                     cbar();
@@ -596,7 +659,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
                             }
                         };
-                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
+                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
                         seq_base += DG::N2 / 2;
                     }
                     cbar();
@@ -631,14 +694,16 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     #pragma unroll
                             for (int nt = 0; nt < NT; ++nt) {
                                 __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS + f;
-                                o[0] = __float2bfloat16_rn(gelu_erf(acc[nt][0] + b0));
-                                o[FS] = __float2bfloat16_rn(gelu_erf(acc[nt][1] + b0));
-                                o[8] = __float2bfloat16_rn(gelu_erf(acc[nt][2] + b1));
-                                o[FS + 8] = __float2bfloat16_rn(gelu_erf(acc[nt][3] + b1));
+                                // exact-erf GELU by the one-ex2 erfc form (fv_device.cuh; erff cost a tenth of the kernel's issue slots)
+                                const uint32_t g0 = gelu_erfc_x2(acc[nt][0] + b0, acc[nt][1] + b0);
+                                const uint32_t g1 = gelu_erfc_x2(acc[nt][2] + b1, acc[nt][3] + b1);
+                                uint16_t* ou = reinterpret_cast<uint16_t*>(o);
+                                ou[0] = (uint16_t)g0; ou[FS] = (uint16_t)(g0 >> 16);
+                                ou[8] = (uint16_t)g1; ou[FS + 8] = (uint16_t)(g1 >> 16);
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
+                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
                             seq_base += DG::N1;
                         } else {
                             gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
@@ -659,7 +724,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] += acc[nt][2] + b1; o[HS + 8] += acc[nt][3] + b1;
                             }
                         };
-                        gemm_ring_kparts<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, D / 16, seq_base, sh_hid, FS, warp, lane, epi);
+                        gemm_ring_kparts<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, D / 16, seq_base, sh_hid, FS, warp, lane, epi);
                         seq_base += DG::N2;
                         cbar();
                     } else {
@@ -673,7 +738,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
+                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
                             seq_base += DG::N2;
                         } else {
                             gemm_rows<4 * D / 16, KS2, NT, NWC, GEMM_MAXL>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);
