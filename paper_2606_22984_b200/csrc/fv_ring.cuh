@@ -108,58 +108,68 @@ __device__ __forceinline__ void st_release_s32(int* p, int v) {
 // The phase is issue-bound (about 25 instructions per row and warp before, two thirds of them the
 // bf16 unpacking and the FMAs): scores and the P V update run on the packed fp32 pipe, even and odd
 // features in the two halves of a register pair, which takes a third of the FMA instructions out.
+template <int D, int DH, int UU>
+__device__ __forceinline__ void attend_rows(const unsigned char* base, int i0, int rows, const uint64_t (&q2)[4], int rg,
+                                            float& m, float& l, uint64_t (&a2)[4]) {
+    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
+    uint4 kk[UU], vv[UU];
+    bool ok[UU];
+#pragma unroll
+    for (int u = 0; u < UU; ++u) {
+        const int row = i0 + u * RPI + rg;
+        ok[u] = row < rows;
+        const unsigned char* p = base + (size_t)(ok[u] ? row : 0) * (4 * D);
+        kk[u] = *reinterpret_cast<const uint4*>(p);
+        vv[u] = *reinterpret_cast<const uint4*>(p + 2 * D);
+    }
+    float s[UU];
+    float mx = m;
+#pragma unroll
+    for (int u = 0; u < UU; ++u) {
+        uint64_t d2 = ffma2(q2[0], bf2_to_f2(kk[u].x), 0ull);
+        d2 = ffma2(q2[1], bf2_to_f2(kk[u].y), d2);
+        d2 = ffma2(q2[2], bf2_to_f2(kk[u].z), d2);
+        d2 = ffma2(q2[3], bf2_to_f2(kk[u].w), d2);
+        float de, dodd;
+        f2unpack(d2, de, dodd);
+        float d = de + dodd;
+#pragma unroll
+        for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+        s[u] = ok[u] ? d : -INFINITY;
+        mx = fmaxf(mx, s[u]);
+    }
+    const float corr = fast_exp2(m - mx);
+    m = mx;
+    l *= corr;
+    const uint64_t c2 = f2pack(corr, corr);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) a2[j] = ffma2(a2[j], c2, 0ull);
+#pragma unroll
+    for (int u = 0; u < UU; ++u) {
+        const float p = fast_exp2(s[u] - mx);
+        l += p;
+        const uint64_t p2 = f2pack(p, p);
+        a2[0] = ffma2(p2, bf2_to_f2(vv[u].x), a2[0]);
+        a2[1] = ffma2(p2, bf2_to_f2(vv[u].y), a2[1]);
+        a2[2] = ffma2(p2, bf2_to_f2(vv[u].z), a2[2]);
+        a2[3] = ffma2(p2, bf2_to_f2(vv[u].w), a2[3]);
+    }
+}
+
+// Full groups of U row sets, then the remaining rows one set (RPI rows) at a time: a ragged tail chunk of two rows
+// costs a quarter of a group instead of a whole one (cfg5: the fifth chunk of every sample holds 2 of 16 rows).
 template <int D, int DH, int CH>
 __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
                                              float& m, float& l, float (&acc)[8]) {
-    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
+    constexpr int LPR = D / 8, RPI = 32 / LPR;
     constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
     const unsigned char* base = chunk + sub * 16;
     const uint64_t q2[4] = {f2pack(q[0], q[1]), f2pack(q[2], q[3]), f2pack(q[4], q[5]), f2pack(q[6], q[7])};
     uint64_t a2[4] = {f2pack(acc[0], acc[1]), f2pack(acc[2], acc[3]), f2pack(acc[4], acc[5]), f2pack(acc[6], acc[7])};
-    for (int i0 = 0; i0 < rows; i0 += RPI * U) {
-        uint4 kk[U], vv[U];
-        bool ok[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int row = i0 + u * RPI + rg;
-            ok[u] = row < rows;
-            const unsigned char* p = base + (size_t)(ok[u] ? row : 0) * (4 * D);
-            kk[u] = *reinterpret_cast<const uint4*>(p);
-            vv[u] = *reinterpret_cast<const uint4*>(p + 2 * D);
-        }
-        float s[U];
-        float mx = m;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            uint64_t d2 = ffma2(q2[0], bf2_to_f2(kk[u].x), 0ull);
-            d2 = ffma2(q2[1], bf2_to_f2(kk[u].y), d2);
-            d2 = ffma2(q2[2], bf2_to_f2(kk[u].z), d2);
-            d2 = ffma2(q2[3], bf2_to_f2(kk[u].w), d2);
-            float de, dodd;
-            f2unpack(d2, de, dodd);
-            float d = de + dodd;
-#pragma unroll
-            for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-            s[u] = ok[u] ? d : -INFINITY;
-            mx = fmaxf(mx, s[u]);
-        }
-        const float corr = fast_exp2(m - mx);
-        m = mx;
-        l *= corr;
-        const uint64_t c2 = f2pack(corr, corr);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) a2[j] = ffma2(a2[j], c2, 0ull);
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const float p = fast_exp2(s[u] - mx);
-            l += p;
-            const uint64_t p2 = f2pack(p, p);
-            a2[0] = ffma2(p2, bf2_to_f2(vv[u].x), a2[0]);
-            a2[1] = ffma2(p2, bf2_to_f2(vv[u].y), a2[1]);
-            a2[2] = ffma2(p2, bf2_to_f2(vv[u].z), a2[2]);
-            a2[3] = ffma2(p2, bf2_to_f2(vv[u].w), a2[3]);
-        }
-    }
+    int i0 = 0;
+    for (; i0 + RPI * U <= rows; i0 += RPI * U) attend_rows<D, DH, U>(base, i0, rows, q2, rg, m, l, a2);
+    if constexpr (U > 1)
+        for (; i0 < rows; i0 += RPI) attend_rows<D, DH, 1>(base, i0, rows, q2, rg, m, l, a2);
 #pragma unroll
     for (int j = 0; j < 4; ++j) f2unpack(a2[j], acc[2 * j], acc[2 * j + 1]);
 }
