@@ -205,7 +205,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     m->mean_nnz = (double)mask_rowptr[N] / N;
     m->device = dev;
     Arena A;
-    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn, img_w1t; };
+    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn, img_w1t, par; };
     const bool lp_tc = !cfg->has_wo && (d == 32 || d == 64 || d == 128);   // fv_logprob.cu path
     const int KP = d < 64 ? 64 : d;
     const int HC = FV_LP_HC;
@@ -263,6 +263,14 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         pack_mma_a(w, d, f, pk.data()); w += (size_t)d * f;
         o.w2 = A.put(pk.data(), (size_t)d * f * 2);
         o.b2 = A.put(w, 4 * d); w += d;
+        {   // the same small parameters once more as one block (layout: fv_internal.h, FvLayerDev::par)
+            std::vector<float> par((size_t)13 * d, 0.f);
+            auto from = [&](size_t off, int n, int at) { std::memcpy(par.data() + at, A.host.data() + off, sizeof(float) * n); };
+            from(o.ln1g, d, 0); from(o.ln1b, d, d); from(o.bqkv, 3 * d, 2 * d);
+            from(o.ln2g, d, 5 * d); from(o.ln2b, d, 6 * d); from(o.b1, f, 7 * d); from(o.b2, d, 11 * d);
+            if (cfg->has_wo) from(o.bo, d, 12 * d);
+            o.par = A.put(par.data(), sizeof(float) * par.size());
+        }
     }
     std::vector<float> wd(d);
     for (int i = 0; i < d; ++i) wd[i] = w[d + i] - w[i];            // head_W[1] - head_W[0]
@@ -392,6 +400,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         L.b2 = (const float*)(base + o.b2);
         L.ln1_g = (const float*)(base + o.ln1g); L.ln1_b = (const float*)(base + o.ln1b);
         L.ln2_g = (const float*)(base + o.ln2g); L.ln2_b = (const float*)(base + o.ln2b);
+        L.par = (const float*)(base + o.par);
         L.img_qkv = lp_tc ? base + o.img_qkv : nullptr;
         L.img_ffn = lp_tc ? base + o.img_ffn : nullptr;
         L.img_w1t = (lp_tc && d == 128) ? base + o.img_w1t : nullptr;

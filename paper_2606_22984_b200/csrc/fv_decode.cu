@@ -54,7 +54,11 @@ struct DecGeo {
                                              : (qkv_bytes > G::hid_bytes ? qkv_bytes : G::hid_bytes));
     static constexpr size_t xa_bytes = CL ? (size_t)R2 * G::AS * 2 : 0;     // LN2 activations of both CTAs (peer-written)
     static constexpr size_t xp_bytes = CL ? (size_t)G::R * G::HS * 4 : 0;   // peer's FFN2 partial sums for my rows
-    static constexpr size_t geo_total = G::total - G::big_bytes - G::split_bytes + big_bytes + split_bytes + xa_bytes + xp_bytes;
+    // the current layer's LayerNorm gains / biases and GEMM biases (FvLayerDev::par), staged by warps that would otherwise
+    // wait: as __ldg operands they cost an L2 round trip in every phase (L1 is ~28 KB next to this carve-out)
+    static constexpr int PAR_E = 5 * D, PAR_L = 8 * D;     // floats used up to the QKV epilogue / after it
+    static constexpr size_t par_bytes = (size_t)(PAR_E + PAR_L) * 4;
+    static constexpr size_t geo_total = G::total - G::big_bytes - G::split_bytes + big_bytes + split_bytes + par_bytes + xa_bytes + xp_bytes;
     static constexpr int CH = fv_ring_ch(D);              // KV rows per ring chunk (host plan agrees)
     static constexpr int ROW_BYTES = 4 * D;               // K[D] | V[D] in bf16
     static constexpr int CHUNK_BYTES = CH * ROW_BYTES;
@@ -226,6 +230,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     // cluster exchange buffers sit at the end of the fixed region (the peer CTA writes them)
     __nv_bfloat16* sh_a2 = reinterpret_cast<__nv_bfloat16*>(smem + DG::fixed - DG::xa_bytes - DG::xp_bytes);
     float* sh_xp = reinterpret_cast<float*>(smem + DG::fixed - DG::xp_bytes);
+    float* sh_par = reinterpret_cast<float*>(smem + DG::fixed - DG::xa_bytes - DG::xp_bytes - DG::par_bytes);
     uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem + DG::fixed);
     uint64_t* bar_empty = bar_full + NSLOT_MAX;
     int* sh_app = reinterpret_cast<int*>(bar_empty + NSLOT_MAX);   // KV appends published so far
@@ -431,6 +436,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     uint32_t seq_base = 0;
     int it = 0;
     const RingCtx rc{ring, bar_full, bar_empty, sh_issued};
+    // sh_par holds: [0, PAR_E) ln1_g | ln1_b | bqkv of the layer about to run (loaded during the attention phase of the
+    // layer before it), [PAR_E, PAR_E + PAR_L) ln2_g | ln2_b | b1 | b2 | bo of the running layer (loaded during its LN1
+    // phase); thread pidx takes float4 number pidx, highest warps first (they have the least other work)
+    const int pidx = NWC * 32 - 1 - tid;
+    if (pidx < DG::PAR_E / 4)
+        reinterpret_cast<float4*>(sh_par)[pidx] = __ldg(reinterpret_cast<const float4*>(m.layer[0].par) + pidx);
     for (int wu = walk0; wu < n_units; wu += n_walk, ++it) {
         const int unit = CL ? wu * 2 + (int)crank : wu;
         const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
@@ -453,14 +464,17 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
             for (int l = 0; l < NL; ++l) {
                 const FvLayerDev& L = m.layer[l];
                 // ---- LN1 (Alg. 2 l.12) -> bf16 activations ----------------------------------
+                float4 pl = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (pidx < DG::PAR_L / 4) pl = __ldg(reinterpret_cast<const float4*>(L.par + DG::PAR_E) + pidx);
                 for (int r = warp; r < R; r += NWC)
-                    ln_row<D>(sh_h + r * HS, L.ln1_g, L.ln1_b, m.ln_eps, false, sh_a + r * AS, lane);
+                    ln_row<D, true>(sh_h + r * HS, sh_par, sh_par + D, m.ln_eps, false, sh_a + r * AS, lane);
+                if (pidx < DG::PAR_L / 4) reinterpret_cast<float4*>(sh_par + DG::PAR_E)[pidx] = pl;
                 cbar();
                 // ---- q, k, v = W a + b (Eq. 2; Alg. 2 l.13) ---------------------------------
                 {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                         const int f = mt * 16 + g;
-                        const float b0 = __ldg(L.bqkv + f), b1 = __ldg(L.bqkv + f + 8);
+                        const float b0 = sh_par[2 * D + f], b1 = sh_par[2 * D + f + 8];
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt) {
                             const int row = nt * 8 + 2 * c4;
@@ -495,6 +509,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 // one step later, so the append shares its barrier with the attention phase and is published
                 // after it
                 asm volatile("fence.proxy.async.global;\n" ::: "memory");
+                float4 pe = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (pidx < DG::PAR_E / 4) pe = __ldg(reinterpret_cast<const float4*>(m.layer[l + 1 < NL ? l + 1 : 0].par) + pidx);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
                 for (int task = warp; task < R * NSPLIT; task += NWC) {
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
@@ -562,6 +578,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 seq_base += (uint32_t)(n_own * nch);
                 if constexpr (DG::WG > 1) seq_base += (uint32_t)((DG::WG - (n_own * nch) % DG::WG) % DG::WG);
+                if (pidx < DG::PAR_E / 4) reinterpret_cast<float4*>(sh_par)[pidx] = pe;
                 cbar();
                 if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
                 if (NSPLIT > 1) {                       // combine the split partials, fixed order
@@ -590,7 +607,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     {
                     auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
-                            const float b0 = __ldg(L.bo + f), b1 = __ldg(L.bo + f + 8);
+                            const float b0 = sh_par[12 * D + f], b1 = sh_par[12 * D + f + 8];
 #pragma unroll
                             for (int nt = 0; nt < NT; ++nt) {
                                 float* o = sh_h + (nt * 8 + 2 * c4) * HS + f;
@@ -615,8 +632,8 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     const uint32_t xpar = (uint32_t)((((long long)it * N + t) * NL + l) & 1);
                     // ---- LN2 of my rows -> my slot of sh_a2, copy to the peer's sh_a2 -------------
                     for (int r = warp; r < R; r += NWC)
-                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1,
-                                  sh_a2 + (crank * R + r) * AS, lane);
+                        ln_row<D, true>(sh_h + r * HS, sh_par + 5 * D, sh_par + 6 * D, m.ln_eps, m.ln2_style == 1,
+                                        sh_a2 + (crank * R + r) * AS, lane);
                     cbar();
                     {
                         constexpr int PCS = R * AS * 2 / 16;            // 16-byte pieces of my R rows
@@ -632,7 +649,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     {
                         auto epi = [&](int mt, int, float (&acc)[NT2][4]) {
                             const int f = mt * 16 + g;
-                            const float b0 = __ldg(L.b1 + crank * 2 * D + f), b1 = __ldg(L.b1 + crank * 2 * D + f + 8);
+                            const float b0 = sh_par[7 * D + crank * 2 * D + f], b1 = sh_par[7 * D + crank * 2 * D + f + 8];
 #pragma unroll
                             for (int nt = 0; nt < NT2; ++nt) {
                                 __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS2 + f;
@@ -678,19 +695,19 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         const int r = i / D, f = i - r * D;
                         const float mine = sh_part[(crank * R + r) * HS + f], theirs = sh_xp[r * HS + f];
                         const float p0 = crank == 0 ? mine : theirs, p1 = crank == 0 ? theirs : mine;
-                        sh_h[r * HS + f] += (p0 + p1) + __ldg(L.b2 + f);
+                        sh_h[r * HS + f] += (p0 + p1) + sh_par[11 * D + f];
                     }
                     cbar();
                 } else {
                     // ---- LN2 (Alg. 2 l.16; ln2_style 1 = Alg. 1 l.5) ----------------------------
                     for (int r = warp; r < R; r += NWC)
-                        ln_row<D>(sh_h + r * HS, L.ln2_g, L.ln2_b, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
+                        ln_row<D, true>(sh_h + r * HS, sh_par + 5 * D, sh_par + 6 * D, m.ln_eps, m.ln2_style == 1, sh_a + r * AS, lane);
                     cbar();
                     // ---- FFN up-projection + exact GELU -> bf16 hidden ---------------------------
                     {
                         auto epi = [&](int mt, int, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
-                            const float b0 = __ldg(L.b1 + f), b1 = __ldg(L.b1 + f + 8);
+                            const float b0 = sh_par[7 * D + f], b1 = sh_par[7 * D + f + 8];
     #pragma unroll
                             for (int nt = 0; nt < NT; ++nt) {
                                 __nv_bfloat16* o = sh_hid + (nt * 8 + 2 * c4) * FS + f;
@@ -716,7 +733,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         // accumulator goes straight into the residual stream
                         auto epi = [&](int mt, float (&acc)[NT][4]) {
                             const int f = mt * 16 + g;
-                            const float b0 = __ldg(L.b2 + f), b1 = __ldg(L.b2 + f + 8);
+                            const float b0 = sh_par[11 * D + f], b1 = sh_par[11 * D + f + 8];
 #pragma unroll
                             for (int nt = 0; nt < NT; ++nt) {
                                 float* o = sh_h + (nt * 8 + 2 * c4) * HS + f;
@@ -746,7 +763,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         cbar();
                         for (int i = tid; i < R * D; i += NWC * 32) {
                             const int r = i / D, f = i - r * D;
-                            float v = __ldg(L.b2 + f);
+                            float v = sh_par[11 * D + f];
 #pragma unroll
                             for (int ks = 0; ks < KS2; ++ks) v += sh_part[((size_t)ks * R + r) * HS + f];
                             sh_h[r * HS + f] += v;

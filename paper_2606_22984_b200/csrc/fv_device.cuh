@@ -175,7 +175,8 @@ __device__ __forceinline__ void gemm_rows(const uint4* __restrict__ wp, int MT, 
 // LayerNorm of one row held in shared memory (fp32), one warp per row: mean, biased variance,
 // eps inside the sqrt, affine (reading A6).  Writes bf16 to `out`; if `replace` the fp32 row is
 // overwritten with the normalised value (ln2_style 1, Alg. 1 l.5).
-template <int D>
+// SM: gam / bet point to shared memory (plain loads) instead of global memory (read-only path).
+template <int D, bool SM = false>
 __device__ __forceinline__ void ln_row(float* hrow, const float* __restrict__ gam, const float* __restrict__ bet,
                                        float eps, bool replace, __nv_bfloat16* out, int lane) {
     constexpr int E = D / 32;
@@ -191,7 +192,7 @@ __device__ __forceinline__ void ln_row(float* hrow, const float* __restrict__ ga
 #pragma unroll
     for (int j = 0; j < E; ++j) {
         const int i = lane * E + j;
-        const float y = (x[j] - mean) * rstd * __ldg(gam + i) + __ldg(bet + i);
+        const float y = SM ? (x[j] - mean) * rstd * gam[i] + bet[i] : (x[j] - mean) * rstd * __ldg(gam + i) + __ldg(bet + i);
         out[i] = __float2bfloat16_rn(y);
         if (replace) hrow[i] = y;
     }

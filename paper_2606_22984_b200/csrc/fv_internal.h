@@ -31,6 +31,9 @@ struct FvLayerDev {
     const uint4* w2;    // [d, 4d]
     const float *bqkv, *bo, *b1, *b2;
     const float *ln1_g, *ln1_b, *ln2_g, *ln2_b;
+    // fv_decode.cu keeps a layer's small fp32 parameters in shared memory; they are copied from this block of 13 d floats:
+    // ln1_g | ln1_b | bqkv (3d) -- used up to the QKV epilogue -- then ln2_g | ln2_b | b1 (4d) | b2 | bo (zeros without W_O)
+    const float* par;
     // fv_logprob.cu: pre-swizzled (SWIZZLE_128B, K-major) bf16 images, copied verbatim into shared memory
     const unsigned char* img_qkv;   // [3d rows x KP]
     const unsigned char* img_ffn;   // per 64-column hidden chunk j: W1_j [64 x KP] | W2_j [d x 64]
