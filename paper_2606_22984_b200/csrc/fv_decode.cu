@@ -102,7 +102,7 @@ __device__ __forceinline__ unsigned char* ring_acquire_w(const RingCtx& rc, uint
 // gemm_rows).  Chunk j of a matrix holds TPCH consecutive 16x16 tiles of its packed image:
 // MPC whole m-tiles when K fits a chunk, else K-part (j % KSP) of m-tile j / KSP.  Warp w
 // consumes chunks w, w + NWC, ... (ring order), A fragments by conflict-free 128-bit LDS.
-template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, class Epi>
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, int EC, class Epi>
 __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32_t seq0, const __nv_bfloat16* act,
                                           int as, int warp, int lane, Epi epi) {
     constexpr bool SPLITK = KT_TOTAL > TPCH;
@@ -144,7 +144,7 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
                 }
             }
         }
-        ring_release(rc, slot, lane);
+        ring_release(rc, slot, lane, EC);
         if constexpr (SPLITK) {
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
@@ -161,7 +161,7 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
 // W2 GEMM (K = 4D > one chunk) with all KSP K-parts of an m-tile consumed by the SAME warp, one after the
 // other (ring order), into one accumulator: no partial-sum buffer and no separate reduction phase --
 // epi(mt, acc) applies bias and residual directly.
-template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, class Epi>
+template <int KT_TOTAL, int NT, int TPCH, int NSLOT, int CHUNK_BYTES, int WG, int EC, class Epi>
 __device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles, uint32_t seq0, const __nv_bfloat16* act,
                                                  int as, int warp, int lane, Epi epi) {
     static_assert(KT_TOTAL % TPCH == 0 && KT_TOTAL > TPCH, "K must span several chunks");
@@ -188,7 +188,7 @@ __device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles
                     mma_bf16(acc[kt & 1][nt], aw, lds32(p), lds32(p + 8));
                 }
             }
-            ring_release(rc, slot, lane);
+            ring_release(rc, slot, lane, EC);
         }
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
@@ -244,7 +244,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
     const int N = m.n_sites, NL = m.n_layers;
 
     if (tid == 0) {
-        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, 1); }
+        // a KV chunk is read by the NSPLIT warps of its sample (each takes its heads): NSPLIT arrivals free a slot;
+        // the one warp that consumes a weight chunk arrives NSPLIT times at once
+        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar_full + i, 1); mbar_init(bar_empty + i, NSPLIT); }
         *sh_app = 0;
         *sh_issued = 0;
         if (CL) { mbar_init(bar_x, NWC); mbar_init(bar_x + 1, NWC); }
@@ -406,7 +408,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 const uint32_t slot = sq % NSLOT, par = (sq / NSLOT) & 1u;
                                 while (!mbar_test(bar_empty + slot, par ^ 1u)) {}
                                 mbar_arrive(bar_full + slot);
-                                mbar_arrive(bar_empty + slot);
+                                mbar_arrive_n(bar_empty + slot, NSPLIT);
                             }
                         __syncwarp();
                         seq += (uint32_t)pad;
@@ -490,7 +492,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                     };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::NQ, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NQ;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wqkv, 3 * D / 16, sh_a, AS, warp, lane, epi);
@@ -512,40 +514,45 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 float4 pe = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (pidx < DG::PAR_E / 4) pe = __ldg(reinterpret_cast<const float4*>(m.layer[l + 1 < NL ? l + 1 : 0].par) + pidx);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
+                // The NSPLIT warps of a sample split the query row by HEADS: warp (r, sp) scores all rows of A(t) against
+                // its D / NSPLIT features and owns the finished output of those heads -- no partial results to merge
+                // between warps, no extra phase; both read every KV chunk of the sample (slots count NSPLIT arrivals).
                 for (int task = warp; task < R * NSPLIT; task += NWC) {
                     const int r = task / NSPLIT, sp = task - r * NSPLIT;
                     if (r >= n_own) continue;
+                    constexpr int DS = D / NSPLIT, LPRS = DS / 8;          // features / lanes of a warp's part of a row
+                    const int rgs = lane / LPRS, subs = lane - rgs * LPRS;
                     const float qs = kLog2e * rsqrtf((float)DH);
-                    const float* qrow = sh_q + r * QS2;
-                    const __nv_bfloat16* kvrow = sh_kv + r * KVS;
+                    const float* qrow = sh_q + r * QS2 + sp * DS;
+                    const __nv_bfloat16* kvrow = sh_kv + r * KVS + sp * DS;
                     float q[8], acc[8];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) q[j] = qrow[sub * 8 + j] * qs;
+                    for (int j = 0; j < 8; ++j) q[j] = qrow[subs * 8 + j] * qs;
                     float mm = -1e30f, ll = 0.f;
 #pragma unroll
                     for (int j = 0; j < 8; ++j) acc[j] = 0.f;
-                    if (sp == 0) {                       // row t itself, as the pool stores it (bf16)
+                    {                                    // row t itself, as the pool stores it (bf16)
                         float d = 0.f;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) d += q[j] * __bfloat162float(kvrow[sub * 8 + j]);
+                        for (int j = 0; j < 8; ++j) d += q[j] * __bfloat162float(kvrow[subs * 8 + j]);
 #pragma unroll
                         for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-                        if (rg == 0) {
+                        if (rgs == 0) {
                             mm = d; ll = 1.f;
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + sub * 8 + j]);
+                            for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + subs * 8 + j]);
                         }
                     }
-                    for (int c = sp; c < nch; c += NSPLIT) {
+                    for (int c = 0; c < nch; ++c) {
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
                         const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
                         uint32_t slot;
                         const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
-                        attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
+                        attend_chunk<D, DH, CH, NSPLIT>(chunk + sp * DS * 2, min(CH, nn - c * CH), q, rgs, subs, mm, ll, acc);
                         ring_release(rc, slot, lane);
                     }
 #pragma unroll
-                    for (int o = LPR; o < 32; o <<= 1) {       // merge the RPI row groups
+                    for (int o = LPRS; o < 32; o <<= 1) {      // merge the row groups of the warp
                         const float m2 = __shfl_xor_sync(0xffffffffu, mm, o);
                         const float l2 = __shfl_xor_sync(0xffffffffu, ll, o);
                         const float mx = fmaxf(mm, m2);
@@ -558,21 +565,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         }
                         mm = mx;
                     }
-                    if (lane < LPR) {
-                        if (NSPLIT > 1) {
-                            float* ps = sh_split + task * SPS;
-                            ps[lane] = mm; ps[LPR + lane] = ll;
+                    if (lane < LPRS) {
+                        const float inv = 1.0f / ll;
+                        if (m.has_wo) {
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) ps[2 * LPR + lane * 8 + j] = acc[j];
+                            for (int j = 0; j < 8; ++j) sh_a[r * AS + sp * DS + lane * 8 + j] = __float2bfloat16_rn(acc[j] * inv);
                         } else {
-                            const float inv = 1.0f / ll;
-                            if (m.has_wo) {
 #pragma unroll
-                                for (int j = 0; j < 8; ++j) sh_a[r * AS + lane * 8 + j] = __float2bfloat16_rn(acc[j] * inv);
-                            } else {
-#pragma unroll
-                                for (int j = 0; j < 8; ++j) sh_h[r * HS + lane * 8 + j] += acc[j] * inv;
-                            }
+                            for (int j = 0; j < 8; ++j) sh_h[r * HS + sp * DS + lane * 8 + j] += acc[j] * inv;
                         }
                     }
                 }
@@ -581,27 +581,6 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 if (pidx < DG::PAR_E / 4) reinterpret_cast<float4*>(sh_par)[pidx] = pe;
                 cbar();
                 if (tid == 0) st_release_s32(sh_app, (it * N + t) * NL + l + 1);
-                if (NSPLIT > 1) {                       // combine the split partials, fixed order
-                    for (int i = tid; i < R * D; i += NWC * 32) {
-                        const int r = i / D, f = i - r * D;
-                        if (r >= n_own) continue;
-                        const float* ps = sh_split + r * NSPLIT * SPS;
-                        float mx = -1e30f;
-#pragma unroll
-                        for (int s = 0; s < NSPLIT; ++s) mx = fmaxf(mx, ps[s * SPS + f / 8]);
-                        float num = 0.f, den = 0.f;
-#pragma unroll
-                        for (int s = 0; s < NSPLIT; ++s) {
-                            const float w = fast_exp2(ps[s * SPS + f / 8] - mx);
-                            den += w * ps[s * SPS + LPR + f / 8];
-                            num += w * ps[s * SPS + 2 * LPR + f];
-                        }
-                        const float u = num / den;
-                        if (m.has_wo) sh_a[r * AS + f] = __float2bfloat16_rn(u);
-                        else sh_h[r * HS + f] += u;
-                    }
-                    cbar();
-                }
                 // ---- optional output projection (bypassed in the paper, l.107) --------------
                 if (m.has_wo) {
                     {
@@ -616,7 +595,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                     if constexpr (DG::WRING) {
-                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::NO, seq_base, sh_a, AS, warp, lane, epi);
                         seq_base += DG::NO;
                     } else {
                         gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.wo, D / 16, sh_a, AS, warp, lane, epi);
@@ -661,7 +640,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 ou[8] = (uint16_t)g1; ou[FS2 + 8] = (uint16_t)(g1 >> 16);
                             }
                         };
-                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
+                        gemm_ring<D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::N1 / 2, seq_base, sh_a2, AS, warp, lane, epi);
                         seq_base += DG::N1 / 2;
                     }
                     cbar();
@@ -676,7 +655,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] = acc[nt][2]; o[HS + 8] = acc[nt][3];
                             }
                         };
-                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
+                        gemm_ring<2 * D / 16, NT2, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::N2 / 2, seq_base, sh_hid, FS2, warp, lane, epi);
                         seq_base += DG::N2 / 2;
                     }
                     cbar();
@@ -720,7 +699,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
+                            gemm_ring<D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::N1, seq_base, sh_a, AS, warp, lane, epi);
                             seq_base += DG::N1;
                         } else {
                             gemm_rows<D / 16, 1, NT, NWC, GEMM_MAXL>(L.w1, 4 * D / 16, sh_a, AS, warp, lane, epi);
@@ -741,7 +720,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                                 o[8] += acc[nt][2] + b1; o[HS + 8] += acc[nt][3] + b1;
                             }
                         };
-                        gemm_ring_kparts<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, D / 16, seq_base, sh_hid, FS, warp, lane, epi);
+                        gemm_ring_kparts<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, D / 16, seq_base, sh_hid, FS, warp, lane, epi);
                         seq_base += DG::N2;
                         cbar();
                     } else {
@@ -755,7 +734,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             }
                         };
                         if constexpr (DG::WRING) {
-                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
+                            gemm_ring<4 * D / 16, NT, DG::TPCH, NSLOT, DG::CHUNK_BYTES, DG::WG, NSPLIT>(rc, DG::N2, seq_base, sh_hid, FS, warp, lane, epi);
                             seq_base += DG::N2;
                         } else {
                             gemm_rows<4 * D / 16, KS2, NT, NWC, GEMM_MAXL>(L.w2, D / 16, sh_hid, FS, warp, lane, epi);

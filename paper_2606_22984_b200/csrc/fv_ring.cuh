@@ -21,6 +21,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_n(uint64_t* bar, uint32_t n) {       // n arrivals at once
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(n) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
@@ -108,10 +111,14 @@ __device__ __forceinline__ void st_release_s32(int* p, int v) {
 // The phase is issue-bound (about 25 instructions per row and warp before, two thirds of them the
 // bf16 unpacking and the FMAs): scores and the P V update run on the packed fp32 pipe, even and odd
 // features in the two halves of a register pair, which takes a third of the FMA instructions out.
-template <int D, int DH, int UU>
+// NS warps share a query row by HEADS (NS = 2: each warp takes D / 2 features, i.e. whole heads, of every row of the
+// chunk -- nothing to merge between the warps afterwards); then LPR = D / 8 / NS lanes cover a warp's part of a row and
+// `base` already points at that part.
+template <int D, int DH, int UU, int NS>
 __device__ __forceinline__ void attend_rows(const unsigned char* base, int i0, int rows, const uint64_t (&q2)[4], int rg,
                                             float& m, float& l, uint64_t (&a2)[4]) {
-    constexpr int LPR = D / 8, RPI = 32 / LPR, LPH = DH / 8;
+    constexpr int LPR = D / 8 / NS, RPI = 32 / LPR, LPH = DH / 8;
+    static_assert(LPR >= LPH && LPR % LPH == 0, "a warp's part of a row holds whole heads");
     uint4 kk[UU], vv[UU];
     bool ok[UU];
 #pragma unroll
@@ -158,18 +165,17 @@ __device__ __forceinline__ void attend_rows(const unsigned char* base, int i0, i
 
 // Full groups of U row sets, then the remaining rows one set (RPI rows) at a time: a ragged tail chunk of two rows
 // costs a quarter of a group instead of a whole one (cfg5: the fifth chunk of every sample holds 2 of 16 rows).
-template <int D, int DH, int CH>
+template <int D, int DH, int CH, int NS = 1>
 __device__ __forceinline__ void attend_chunk(const unsigned char* chunk, int rows, const float (&q)[8], int rg, int sub,
                                              float& m, float& l, float (&acc)[8]) {
-    constexpr int LPR = D / 8, RPI = 32 / LPR;
-    constexpr int ITER = CH / RPI, U = ITER < 4 ? ITER : 4;
+    constexpr int LPR = D / 8 / NS, RPI = 32 / LPR;
+    constexpr int ITER = (CH + RPI - 1) / RPI, U = ITER < 4 ? ITER : 4;
     const unsigned char* base = chunk + sub * 16;
     const uint64_t q2[4] = {f2pack(q[0], q[1]), f2pack(q[2], q[3]), f2pack(q[4], q[5]), f2pack(q[6], q[7])};
     uint64_t a2[4] = {f2pack(acc[0], acc[1]), f2pack(acc[2], acc[3]), f2pack(acc[4], acc[5]), f2pack(acc[6], acc[7])};
     int i0 = 0;
-    for (; i0 + RPI * U <= rows; i0 += RPI * U) attend_rows<D, DH, U>(base, i0, rows, q2, rg, m, l, a2);
-    if constexpr (U > 1)
-        for (; i0 < rows; i0 += RPI) attend_rows<D, DH, 1>(base, i0, rows, q2, rg, m, l, a2);
+    for (; i0 + RPI * U <= rows; i0 += RPI * U) attend_rows<D, DH, U, NS>(base, i0, rows, q2, rg, m, l, a2);
+    for (; i0 < rows; i0 += RPI) attend_rows<D, DH, 1, NS>(base, i0, rows, q2, rg, m, l, a2);
 #pragma unroll
     for (int j = 0; j < 4; ++j) f2unpack(a2[j], acc[2 * j], acc[2 * j + 1]);
 }
@@ -211,13 +217,13 @@ __device__ __forceinline__ unsigned char* ring_acquire(const RingCtx& rc, uint32
     mbar_wait(rc.bar_full + slot, par);
     return rc.ring + (size_t)slot * CHUNK_BYTES;
 }
-__device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane) {
+__device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, int lane, uint32_t arrivals = 1) {
     // The slot is refilled by cp.async.bulk (async proxy): order this warp's generic-proxy reads of
     // it before that write.  Without the fence a refill could overtake the reads (seen as run-to-run
     // differences of ~1e-4 in both samples of a CTA at one step, 15 of 16 fresh-model runs).
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
     __syncwarp();
-    if (lane == 0) mbar_arrive(rc.bar_empty + slot);
+    if (lane == 0) mbar_arrive_n(rc.bar_empty + slot, arrivals);
 }
 
 }  // namespace fvring
