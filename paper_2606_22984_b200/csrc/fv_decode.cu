@@ -331,6 +331,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
             const int unit = CL ? wu * 2 + (int)crank : wu;
             const int b_first = unit < a.n_groups ? unit * a.rows_per_group : 0;
             const int n_own = unit < a.n_groups ? min(a.rows_per_group, a.B - b_first) : 0;   // 0: FFN helper only
+            const uint32_t inv_own = n_own > 0 ? (65536u + (uint32_t)n_own - 1u) / (uint32_t)n_own : 0u;
             // copy plan of a step: chunk -> run list (staged in shared memory when it fits)
             struct Plan { int nch, nn, nruns; const int32_t* cptr; const int2* rptr; };
             auto stage_plan = [&](int t) {
@@ -380,9 +381,12 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             // chunk-major inside a round of GR samples (= the samples the compute
                             // warps work on at the same time), rounds in order: every warp then
                             // consumes its chunks in ring order
-                            const int k = i / (GR * nch), rem = i - k * GR * nch;
-                            const int nk = min(GR, n_own - k * GR);
-                            const int c = rem / nk;
+                            // (one round when all rows are attended at once; then c = i / n_own by multiply and shift,
+                            // exact below 2048 for divisors up to 32 -- two integer divisions were a fifth of a round)
+                            int k = 0, rem = i;
+                            if constexpr (R > GR) { k = i / (GR * nch); rem = i - k * GR * nch; }
+                            const int nk = R > GR ? min(GR, n_own - k * GR) : n_own;
+                            const int c = (R <= GR && total < 2048) ? (int)(((uint32_t)rem * inv_own) >> 16) : rem / nk;
                             const int r = k * GR + (rem - c * nk);
                             const int rows = min(CH, nn - c * CH);
                             mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * DG::ROW_BYTES);
