@@ -504,17 +504,24 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                 }
                 cbar();
                 // ---- append k_t, v_t to the KV pool as bf16 (Alg. 2 l.17; reading A2) -------
-                for (int i = tid; i < R * (2 * D / 8); i += NWC * 32) {
-                    const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
-                    if (r >= n_own) continue;
-                    const uint4 v = *reinterpret_cast<const uint4*>(sh_kv + r * KVS + ch * 8);
-                    __nv_bfloat16* dst = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + t % m.kv_rows) * (2 * D) + ch * 8;
-                    *reinterpret_cast<uint4*>(dst) = v;
+                // The warps without an attention task (sample slots the CTA does not own: 2 of 16 warps at 7 samples) take
+                // the whole append and its proxy fence off the others' path to their first KV chunk; with every slot owned
+                // all threads share it.  The producer reads these rows through the async proxy (cp.async.bulk); they are
+                // first needed one step later, so the append shares its barrier with the attention phase and is
+                // published after it.
+                {
+                    const int busy = n_own * NSPLIT < NWC ? n_own * NSPLIT : 0;       // warps below `busy` skip the append
+                    if (warp >= busy) {
+                        for (int i = tid - busy * 32; i < R * (2 * D / 8); i += (NWC - busy) * 32) {
+                            const int r = i / (2 * D / 8), ch = i - r * (2 * D / 8);
+                            if (r >= n_own) continue;
+                            const uint4 v = *reinterpret_cast<const uint4*>(sh_kv + r * KVS + ch * 8);
+                            __nv_bfloat16* dst = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + t % m.kv_rows) * (2 * D) + ch * 8;
+                            *reinterpret_cast<uint4*>(dst) = v;
+                        }
+                        asm volatile("fence.proxy.async.global;\n" ::: "memory");
+                    }
                 }
-                // the producer reads these rows through the async proxy (cp.async.bulk); they are first needed
-                // one step later, so the append shares its barrier with the attention phase and is published
-                // after it
-                asm volatile("fence.proxy.async.global;\n" ::: "memory");
                 float4 pe = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (pidx < DG::PAR_E / 4) pe = __ldg(reinterpret_cast<const float4*>(m.layer[l + 1 < NL ? l + 1 : 0].par) + pidx);
                 // ---- masked attention from the KV ring + residual (Eq. 3; Alg. 2 l.14-15) ---
