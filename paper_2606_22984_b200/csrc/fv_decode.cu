@@ -144,7 +144,14 @@ __device__ __forceinline__ void gemm_ring(const RingCtx& rc, int nchunks, uint32
                 }
             }
         }
-        ring_release(rc, slot, lane, EC);
+        {   // every A fragment read from the slot has fed an MMA of one of these accumulators
+            uint32_t h = 0;
+#pragma unroll
+            for (int q = 0; q < NCH; ++q)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) h ^= __float_as_uint(acc[q][nt][0]);
+            ring_release_dep(rc, slot, lane, EC, h);
+        }
         if constexpr (SPLITK) {
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
@@ -188,7 +195,12 @@ __device__ __forceinline__ void gemm_ring_kparts(const RingCtx& rc, int n_mtiles
                     mma_bf16(acc[kt & 1][nt], aw, lds32(p), lds32(p + 8));
                 }
             }
-            ring_release(rc, slot, lane, EC);
+            {
+                uint32_t h = 0;
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) h ^= __float_as_uint(acc[0][nt][0]) ^ __float_as_uint(acc[1][nt][0]);
+                ring_release_dep(rc, slot, lane, EC, h);
+            }
         }
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
@@ -560,7 +572,9 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         uint32_t slot;
                         const unsigned char* chunk = ring_acquire<NSLOT, DG::CHUNK_BYTES>(rc, sq, slot);
                         attend_chunk<D, DH, CH, NSPLIT>(chunk + sp * DS * 2, min(CH, nn - c * CH), q, rgs, subs, mm, ll, acc);
-                        ring_release(rc, slot, lane);
+                        // every K word fed the scores behind ll, V words x / y / z / w fed acc[0..1] / [2..3] / [4..5] / [6..7]
+                        ring_release_dep(rc, slot, lane, 1, __float_as_uint(ll) ^ __float_as_uint(acc[0]) ^ __float_as_uint(acc[2]) ^
+                                                                __float_as_uint(acc[4]) ^ __float_as_uint(acc[6]));
                     }
 #pragma unroll
                     for (int o = LPRS; o < 32; o <<= 1) {      // merge the row groups of the warp

@@ -226,4 +226,17 @@ __device__ __forceinline__ void ring_release(const RingCtx& rc, uint32_t slot, i
     if (lane == 0) mbar_arrive_n(rc.bar_empty + slot, arrivals);
 }
 
+// The same release without the proxy fence, for a warp whose reads of the slot have all been CONSUMED: `h` must be computed
+// (in every lane) from results of arithmetic that used every value the lane loaded from the slot.  The hazard the fence
+// guards against is the arrive (issued to the barrier unit, SYNCS) overtaking shared-memory loads still in flight, so that
+// the refill lands before they are performed; a load whose value has been used is performed.  The vote cannot issue before
+// h is ready in all lanes and the arrive takes its count from the vote's result, so the arrive issues after every such
+// load has returned -- in SASS, not only in program order (the compare is never true in practice and both counts are equal).
+__device__ __forceinline__ void ring_release_dep(const RingCtx& rc, uint32_t slot, int lane, uint32_t arrivals, uint32_t h) {
+    uint32_t same;
+    asm volatile("mov.u32 %0, %1;" : "=r"(same) : "r"(arrivals));
+    const bool never = __any_sync(0xffffffffu, h == 0x9E3779B9u);
+    if (lane == 0) mbar_arrive_n(rc.bar_empty + slot, never ? arrivals : same);
+}
+
 }  // namespace fvring
