@@ -291,6 +291,7 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     bool band = band_w >= 1 && 2 * (band_w + 1) <= N;
     for (int t = 0; t < N && band; ++t)
         band = mask_col[mask_rowptr[t]] == std::max(0, t - band_w) && mask_rowptr[t + 1] - mask_rowptr[t] == t - mask_col[mask_rowptr[t]] + 1;
+    const bool band_shape = band;      // (the copy plans must not depend on the pool the environment picks)
     if (const char* kvm = std::getenv("FLASHVAN_KV"); kvm && std::strcmp(kvm, "dense") == 0) band = false;
     const int kv_rows = band ? band_w + 1 : N;
     m->window = band ? kv_rows : 0;
@@ -312,6 +313,34 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         chunk_ptr[t + 1] = (int32_t)chunk_run_ptr.size() - 1;
     }
     if (runs.empty()) runs.push_back(make_int2(0, 0));
+    // plan of fv_decode.cu (fv_internal.h: d_*): isolated positions first taken out, then the same chunking
+    std::vector<int32_t> d_chunk_ptr(N + 1, 0), d_chunk_run_ptr(1, 0), d_nn(N, 0), d_dir((size_t)N * FV_DIRECT_MAX, -1);
+    std::vector<int2> d_runs;
+    for (int t = 0; t < N; ++t) {
+        const int e0 = mask_rowptr[t], nn = mask_rowptr[t + 1] - 1 - e0;
+        std::vector<int32_t> st;                                   // positions that stream through the ring
+        int nd = 0;
+        for (int i = 0; i < nn; ++i) {
+            const int p0 = mask_col[e0 + i];
+            const bool alone = (i == 0 || mask_col[e0 + i - 1] != p0 - 1) && (i + 1 == nn || mask_col[e0 + i + 1] != p0 + 1);
+            if (alone && nd < FV_DIRECT_MAX && d <= 128 && !band_shape) d_dir[(size_t)t * FV_DIRECT_MAX + nd++] = p0 % kv_rows;
+            else st.push_back(p0);
+        }
+        const int ns = (int)st.size();
+        d_nn[t] = ns;
+        for (int c0 = 0; c0 < ns; c0 += CH) {
+            const int rows = std::min(CH, ns - c0);
+            for (int i = 0; i < rows;) {
+                int j = i + 1;
+                while (j < rows && st[c0 + j] == st[c0 + j - 1] + 1 && st[c0 + j] % kv_rows != 0) ++j;
+                d_runs.push_back(make_int2(st[c0 + i] % kv_rows, (i << 16) | (j - i)));
+                i = j;
+            }
+            d_chunk_run_ptr.push_back((int32_t)d_runs.size());
+        }
+        d_chunk_ptr[t + 1] = (int32_t)d_chunk_run_ptr.size() - 1;
+    }
+    if (d_runs.empty()) d_runs.push_back(make_int2(0, 0));
     // block attention plan of fv_logprob.cu: union of the key positions of 32 consecutive mask rows
     const int BQ = 32;
     const int n_blk = (N + BQ - 1) / BQ;
@@ -341,6 +370,11 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     const size_t o_cp = A.put(chunk_ptr.data(), sizeof(int32_t) * chunk_ptr.size());
     const size_t o_crp = A.put(chunk_run_ptr.data(), sizeof(int32_t) * chunk_run_ptr.size());
     const size_t o_runs = A.put(runs.data(), sizeof(int2) * runs.size());
+    const size_t o_dcp = A.put(d_chunk_ptr.data(), sizeof(int32_t) * d_chunk_ptr.size());
+    const size_t o_dcrp = A.put(d_chunk_run_ptr.data(), sizeof(int32_t) * d_chunk_run_ptr.size());
+    const size_t o_druns = A.put(d_runs.data(), sizeof(int2) * d_runs.size());
+    const size_t o_dnn = A.put(d_nn.data(), sizeof(int32_t) * d_nn.size());
+    const size_t o_ddir = A.put(d_dir.data(), sizeof(int32_t) * d_dir.size());
 
     m->arena_bytes = A.host.size();
     e = cudaMalloc(&m->arena, m->arena_bytes);
@@ -378,6 +412,11 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     D.chunk_ptr = (const int32_t*)(base + o_cp);
     D.chunk_run_ptr = (const int32_t*)(base + o_crp);
     D.runs = (const int2*)(base + o_runs);
+    D.d_chunk_ptr = (const int32_t*)(base + o_dcp);
+    D.d_chunk_run_ptr = (const int32_t*)(base + o_dcrp);
+    D.d_runs = (const int2*)(base + o_druns);
+    D.d_nn = (const int32_t*)(base + o_dnn);
+    D.d_dir = (const int32_t*)(base + o_ddir);
     D.att_blk_uptr = (const int32_t*)(base + o_bu);
     D.att_ukeys = (const int32_t*)(base + o_uk);
     D.att_mask = (const uint16_t*)(base + o_am);

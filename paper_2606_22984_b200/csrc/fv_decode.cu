@@ -349,21 +349,21 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
             auto stage_plan = [&](int t) {
                 Plan p;
                 if (t >= N) { p.nch = p.nn = p.nruns = 0; p.cptr = nullptr; p.rptr = nullptr; return p; }
-                const int cp0 = __ldg(m.chunk_ptr + t);
-                p.nch = __ldg(m.chunk_ptr + t + 1) - cp0;
-                p.nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
-                const int rp0 = __ldg(m.chunk_run_ptr + cp0);
-                p.nruns = __ldg(m.chunk_run_ptr + cp0 + p.nch) - rp0;
+                const int cp0 = __ldg(m.d_chunk_ptr + t);
+                p.nch = __ldg(m.d_chunk_ptr + t + 1) - cp0;
+                p.nn = __ldg(m.d_nn + t);
+                const int rp0 = __ldg(m.d_chunk_run_ptr + cp0);
+                p.nruns = __ldg(m.d_chunk_run_ptr + cp0 + p.nch) - rp0;
                 int32_t* tc = tab_c + (t & 1) * DG::TAB_C;
                 int2* tr = tab_r + (t & 1) * DG::TAB_R;
                 __syncwarp();
                 if (p.nch + 1 <= DG::TAB_C && p.nruns <= DG::TAB_R) {
-                    for (int i = lane; i <= p.nch; i += 32) tc[i] = __ldg(m.chunk_run_ptr + cp0 + i) - rp0;
-                    for (int i = lane; i < p.nruns; i += 32) tr[i] = __ldg(m.runs + rp0 + i);
+                    for (int i = lane; i <= p.nch; i += 32) tc[i] = __ldg(m.d_chunk_run_ptr + cp0 + i) - rp0;
+                    for (int i = lane; i < p.nruns; i += 32) tr[i] = __ldg(m.d_runs + rp0 + i);
                     __syncwarp();
                     p.cptr = tc; p.rptr = tr;
                 } else {
-                    p.cptr = m.chunk_run_ptr + cp0; p.rptr = m.runs;      // absolute run indices
+                    p.cptr = m.d_chunk_run_ptr + cp0; p.rptr = m.d_runs;      // absolute run indices
                 }
                 return p;
             };
@@ -467,8 +467,11 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
         if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
         for (int t = 0; t < N; ++t) {
             const int me0 = __ldg(m.mask_rowptr + t);
-            const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
+            const int nn = __ldg(m.d_nn + t);                        // rows that come through the ring
             const int nch = (nn + CH - 1) / CH;
+            int dir_pos[FV_DIRECT_MAX];                              // isolated key positions, loaded straight from the pool
+#pragma unroll
+            for (int i = 0; i < FV_DIRECT_MAX; ++i) dir_pos[i] = __ldg(m.d_dir + (size_t)t * FV_DIRECT_MAX + i);
             if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
             cbar();
             // ---- concatenated positional embedding (Eq. 15, l.287-292) -------------------
@@ -566,6 +569,17 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + subs * 8 + j]);
                         }
                     }
+                    // row group g < FV_DIRECT_MAX requests the step's g-th isolated row now and uses it after the ring's rows
+                    // (written by this CTA in an earlier step, plain stores; barriers since)
+                    uint4 dk = make_uint4(0u, 0u, 0u, 0u), dv = dk;
+                    int dpos = -1;
+#pragma unroll
+                    for (int i = 0; i < FV_DIRECT_MAX; ++i) if (rgs == i) dpos = dir_pos[i];
+                    if (dpos >= 0) {
+                        const __nv_bfloat16* dp = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + dpos) * (2 * D) + sp * DS + subs * 8;
+                        dk = *reinterpret_cast<const uint4*>(dp);
+                        dv = *reinterpret_cast<const uint4*>(dp + D);
+                    }
                     for (int c = 0; c < nch; ++c) {
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
                         const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
@@ -576,6 +590,7 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         ring_release_dep(rc, slot, lane, 1, __float_as_uint(ll) ^ __float_as_uint(acc[0]) ^ __float_as_uint(acc[2]) ^
                                                                 __float_as_uint(acc[4]) ^ __float_as_uint(acc[6]));
                     }
+                    if (dir_pos[0] >= 0) attend_direct<DH>(dk, dv, dpos >= 0, q, mm, ll, acc);
 #pragma unroll
                     for (int o = LPRS; o < 32; o <<= 1) {      // merge the row groups of the warp
                         const float m2 = __shfl_xor_sync(0xffffffffu, mm, o);

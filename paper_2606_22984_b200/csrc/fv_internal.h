@@ -19,6 +19,7 @@ constexpr int FV_LP_HC = 64;
 #ifndef FV_DEC_CH128
 #define FV_DEC_CH128 16
 #endif
+#define FV_DIRECT_MAX 2
 constexpr int fv_ring_ch(int d_model) { return d_model >= 256 ? 8 : (d_model >= 128 ? FV_DEC_CH128 : 16); }
 
 // Per-layer device pointers.  GEMM weights are bf16, pre-packed at fv_create_model time into
@@ -59,6 +60,14 @@ struct FvModelDev {
     const int32_t* chunk_ptr;      // [N+1]  chunks before step t
     const int32_t* chunk_run_ptr;  // [n_chunks+1]
     const int2* runs;
+    // fv_decode.cu's own copy plan: the same, built without the step's first FV_DIRECT_MAX ISOLATED key positions (runs of
+    // one row, e.g. the lattice neighbour two rows up) -- those rows the attention warps load straight from the pool, which
+    // takes one small bulk copy per sample and layer-step off the TMA unit that paces the attention phase.
+    const int32_t* d_chunk_ptr;    // [N+1]
+    const int32_t* d_chunk_run_ptr;
+    const int2* d_runs;
+    const int32_t* d_nn;           // [N]  rows of step t that come through the ring
+    const int32_t* d_dir;          // [N * FV_DIRECT_MAX]  physical rows loaded directly, -1 = none
     __nv_bfloat16* kv;      // [max_batch][n_layers][N][2d]  (K row then V row, bf16); fv_log_prob's pool
     // fv_sample's pool: the same array, or -- when every mask row is one run t-W..t (the band of Eq. S1) --
     // a ring-buffer window [max_batch][n_layers][kv_rows = W+1][2d] in which position p lives in row p % kv_rows

@@ -163,6 +163,34 @@ __device__ __forceinline__ void attend_rows(const unsigned char* base, int i0, i
     }
 }
 
+// The same update with ONE row per row group whose K / V words the lane already holds in registers (rows fv_decode.cu
+// loads straight from the pool; `ok` false = this row group has none).
+template <int DH>
+__device__ __forceinline__ void attend_direct(const uint4& kk, const uint4& vv, bool ok, const float (&q)[8],
+                                              float& m, float& l, float (&acc)[8]) {
+    constexpr int LPH = DH / 8;
+    uint64_t d2 = ffma2(f2pack(q[0], q[1]), bf2_to_f2(kk.x), 0ull);
+    d2 = ffma2(f2pack(q[2], q[3]), bf2_to_f2(kk.y), d2);
+    d2 = ffma2(f2pack(q[4], q[5]), bf2_to_f2(kk.z), d2);
+    d2 = ffma2(f2pack(q[6], q[7]), bf2_to_f2(kk.w), d2);
+    float de, dodd;
+    f2unpack(d2, de, dodd);
+    float d = de + dodd;
+#pragma unroll
+    for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
+    const float s = ok ? d : -INFINITY;
+    const float mx = fmaxf(m, s);
+    const float corr = fast_exp2(m - mx), p = fast_exp2(s - mx);
+    m = mx;
+    l = l * corr + p;
+    const uint32_t w[4] = {vv.x, vv.y, vv.z, vv.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        acc[2 * j] = acc[2 * j] * corr + p * bf_lo(w[j]);
+        acc[2 * j + 1] = acc[2 * j + 1] * corr + p * bf_hi(w[j]);
+    }
+}
+
 // Full groups of U row sets, then the remaining rows one set (RPI rows) at a time: a ragged tail chunk of two rows
 // costs a quarter of a group instead of a whole one (cfg5: the fifth chunk of every sample holds 2 of 16 rows).
 template <int D, int DH, int CH, int NS = 1>
