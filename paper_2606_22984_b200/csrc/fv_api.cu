@@ -326,6 +326,12 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
             if (alone && nd < FV_DIRECT_MAX && d <= 128 && !band_shape) d_dir[(size_t)t * FV_DIRECT_MAX + nd++] = p0 % kv_rows;
             else st.push_back(p0);
         }
+        // a ragged tail of the ring's rows that still fits the direct slots goes the same way (cfg5: 65 = 4 x 16 + 1 rows:
+        // no fifth chunk of one row per sample)
+        if (const int rem = (int)st.size() % CH; rem > 0 && rem <= FV_DIRECT_MAX - nd && d <= 128 && !band_shape) {
+            for (int i = 0; i < rem; ++i) d_dir[(size_t)t * FV_DIRECT_MAX + nd++] = st[st.size() - rem + i] % kv_rows;
+            st.resize(st.size() - rem);
+        }
         const int ns = (int)st.size();
         d_nn[t] = ns;
         for (int c0 = 0; c0 < ns; c0 += CH) {
