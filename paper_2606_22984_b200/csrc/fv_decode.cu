@@ -552,21 +552,26 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                     const float* qrow = sh_q + r * QS2 + sp * DS;
                     const __nv_bfloat16* kvrow = sh_kv + r * KVS + sp * DS;
                     float q[8], acc[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) q[j] = qrow[subs * 8 + j] * qs;
+                    {                                    // (rows are 16-byte aligned: QS2, KVS and the offsets are multiples of 16 B)
+                        const float4 qa = *reinterpret_cast<const float4*>(qrow + subs * 8), qb = *reinterpret_cast<const float4*>(qrow + subs * 8 + 4);
+                        q[0] = qa.x * qs; q[1] = qa.y * qs; q[2] = qa.z * qs; q[3] = qa.w * qs;
+                        q[4] = qb.x * qs; q[5] = qb.y * qs; q[6] = qb.z * qs; q[7] = qb.w * qs;
+                    }
                     float mm = -1e30f, ll = 0.f;
 #pragma unroll
                     for (int j = 0; j < 8; ++j) acc[j] = 0.f;
                     {                                    // row t itself, as the pool stores it (bf16)
+                        const uint4 ks = *reinterpret_cast<const uint4*>(kvrow + subs * 8), vs = *reinterpret_cast<const uint4*>(kvrow + D + subs * 8);
+                        const uint32_t kw[4] = {ks.x, ks.y, ks.z, ks.w}, vw[4] = {vs.x, vs.y, vs.z, vs.w};
                         float d = 0.f;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) d += q[j] * __bfloat162float(kvrow[subs * 8 + j]);
+                        for (int j = 0; j < 4; ++j) { d += q[2 * j] * bf_lo(kw[j]); d += q[2 * j + 1] * bf_hi(kw[j]); }
 #pragma unroll
                         for (int o = 1; o < LPH; o <<= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
                         if (rgs == 0) {
                             mm = d; ll = 1.f;
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + subs * 8 + j]);
+                            for (int j = 0; j < 4; ++j) { acc[2 * j] = bf_lo(vw[j]); acc[2 * j + 1] = bf_hi(vw[j]); }
                         }
                     }
                     // row group g < FV_DIRECT_MAX requests the step's g-th isolated row now and uses it after the ring's rows
