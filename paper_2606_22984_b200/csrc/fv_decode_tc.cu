@@ -196,6 +196,11 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
                 const Plan nxt = stage_plan(t + 1);
                 const int nch = cur.nch, nn = cur.nn;
                 const int total = n_own * nch;
+                // chunk index -> (round, chunk, sample) without integer divisions in the per-lane path (they showed in the
+                // kernel time of fv_decode.cu): q = umulhi(i, ceil(2^32 / d)) is exact for i, d < 2^16
+                const uint32_t d_round = (uint32_t)(GR * (nch > 0 ? nch : 1)), inv_round = (uint32_t)((0x100000000ull + d_round - 1) / d_round);
+                const uint32_t nk0 = (uint32_t)min(GR, n_own > 0 ? n_own : 1), inv_nk0 = (uint32_t)((0x100000000ull + nk0 - 1) / nk0);
+                const uint32_t nk1 = (uint32_t)(n_own > GR ? n_own - GR : 1), inv_nk1 = (uint32_t)((0x100000000ull + nk1 - 1) / nk1);
                 for (int l = 0; l < NL; ++l) {
                     const FvLayerDev& L = m.layer[l];
                     // W_qkv tile i = (M-tile i / 2, K-block i % 2) of the [3d x d] image: K-block slabs of 384 rows
@@ -213,9 +218,14 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
                         const unsigned int bm = __ballot_sync(0xffffffffu, ok);
                         const int npre = bm == 0xffffffffu ? 32 : __ffs(~bm) - 1;
                         if (lane < npre) {
-                            const int k = i / (GR * nch), rem = i - k * GR * nch;      // chunk-major inside a round of GR samples
+                            // chunk-major inside a round of GR samples
+                            const bool small = total < 65536;
+                            const int k = small ? (d_round == 1u ? i : (int)__umulhi((uint32_t)i, inv_round)) : i / (GR * nch);
+                            const int rem = i - k * GR * nch;
                             const int nk = min(GR, n_own - k * GR);
-                            const int c = rem / nk;
+                            const int c = !small ? rem / nk
+                                                 : (k == 0 ? (nk0 == 1u ? rem : (int)__umulhi((uint32_t)rem, inv_nk0))
+                                                           : (nk1 == 1u ? rem : (int)__umulhi((uint32_t)rem, inv_nk1)));
                             const int r = k * GR + (rem - c * nk);
                             const int rows = min(CH, nn - c * CH);
                             mbar_arrive_expect_tx(bar_full + slot, (uint32_t)rows * ROW_BYTES);
