@@ -386,7 +386,10 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
                         uint32_t slot;
                         const unsigned char* chunk = ring_acquire<NSLOT, CHUNK_BYTES>(rc, sq, slot);
                         attend_chunk<D, DH, CH>(chunk, min(CH, nn - c * CH), q, rg, sub, mm, ll, acc);
-                        ring_release(rc, slot, lane);
+                        // release by data dependency instead of a proxy fence (fv_ring.cuh): every K word fed the scores behind
+                        // ll, the V words fed acc[0..1] / [2..3] / [4..5] / [6..7]
+                        ring_release_dep(rc, slot, lane, 1, __float_as_uint(ll) ^ __float_as_uint(acc[0]) ^ __float_as_uint(acc[2]) ^
+                                                                __float_as_uint(acc[4]) ^ __float_as_uint(acc[6]));
                     }
 #pragma unroll
                     for (int o = LPR; o < 32; o <<= 1) {       // merge the row groups of the warp
