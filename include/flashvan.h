@@ -95,8 +95,8 @@ int fv_sample(fv_model* m, int32_t B, const float* uniforms, int8_t* spins, floa
  *   spins [device] [B,N] int8 in (+-1; other values are undefined behaviour).
  *   (vocab > 2: token ids as unsigned bytes, cond_p = probability of the given token.)
  *   logq, cond_p as in fv_sample.  Overwrites the model's KV pool and workspace: calls on one model
- *   must be ordered on one stream.  Enqueues 3 * n_layers + 1 kernels (layer-major tensor-core path) or
- *   one (chunked teacher forcing: d_model = 256 or has_wo). */
+ *   must be ordered on one stream.  Enqueues 3 * n_layers + 1 kernels (layer-major tensor-core path; 4 * n_layers + 1
+ *   with has_wo: the out-projection is one more tcgen05 GEMM per layer) or one (chunked teacher forcing: d_model = 256). */
 int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float* cond_p,
                 void* stream);
 
@@ -109,7 +109,7 @@ int fv_log_prob(fv_model* m, int32_t B, const int8_t* spins, float* logq, float*
  * call on a device looks the array's address up once (cudaGetSymbolAddress).
  *   Limit: B * N * d_model * (8 + 4 * n_layers) bytes (+ alignment) <= FV_STATIC_SCRATCH_BYTES, i.e. 16 384 rows
  *   (B * N) for a 6-layer d_model = 128 model; larger calls return FV_ERR_BAD_ARG and fv_last_error() names the
- *   bytes needed.  Shapes the layer-major path does not cover (has_wo, d_model = 256) return FV_ERR_BAD_SHAPE.
+ *   bytes needed.  Shapes the layer-major path does not cover (d_model = 256) return FV_ERR_BAD_SHAPE.
  *   The array is shared by every model and every call on the device and keeps the previous call's contents; nothing
  *   in it needs clearing (each call writes every row before reading it), but two calls that overlap on the GPU
  *   (different streams, or two host threads) race on it: order them on one stream.  The model's KV pool is untouched.

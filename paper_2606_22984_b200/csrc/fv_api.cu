@@ -205,8 +205,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
     m->mean_nnz = (double)mask_rowptr[N] / N;
     m->device = dev;
     Arena A;
-    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn, img_w1t, par; };
-    const bool lp_tc = !cfg->has_wo && (d == 32 || d == 64 || d == 128);   // fv_logprob.cu path
+    struct Off { size_t wqkv, wo, w1, w2, bqkv, bo, b1, b2, ln1g, ln1b, ln2g, ln2b, img_qkv, img_ffn, img_w1t, img_wo, par; };
+    const bool lp_tc = d == 32 || d == 64 || d == 128;                     // fv_logprob.cu path
     const int KP = d < 64 ? 64 : d;
     const int HC = FV_LP_HC;
     std::vector<uint16_t> img((size_t)std::max(3 * d * KP, (f / HC) * (HC * KP + d * HC)));
@@ -234,7 +234,12 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         }
         o.bqkv = A.put(tb.data(), 4 * 3 * d);
         o.wo = o.bo = 0;
+        o.img_wo = 0;
         if (cfg->has_wo) {
+            if (lp_tc) {
+                fv_pack_sw128(w, d, d, d, KP, img.data());
+                o.img_wo = A.put(img.data(), (size_t)d * KP * 2);
+            }
             pack_mma_a(w, d, d, pk.data()); w += (size_t)d * d;
             o.wo = A.put(pk.data(), (size_t)d * d * 2);
             o.bo = A.put(w, 4 * d); w += d;
@@ -448,7 +453,8 @@ int fv_create_model(const fv_config* cfg, const float* weights, int64_t n_weight
         L.par = (const float*)(base + o.par);
         L.img_qkv = lp_tc ? base + o.img_qkv : nullptr;
         L.img_ffn = lp_tc ? base + o.img_ffn : nullptr;
-        L.img_w1t = (lp_tc && d == 128) ? base + o.img_w1t : nullptr;
+        L.img_w1t = (lp_tc && d == 128 && !cfg->has_wo) ? base + o.img_w1t : nullptr;
+        L.img_wo = (lp_tc && cfg->has_wo) ? base + o.img_wo : nullptr;
     }
     *out = m;
     return FV_OK;
@@ -613,8 +619,8 @@ int fv_log_prob_static(fv_model* m, int32_t B, const int8_t* spins, float* logq,
     if (!m || !spins || !logq) return fail(FV_ERR_BAD_ARG, "null argument");
     if (B <= 0) return fail(FV_ERR_BAD_ARG, "B must be positive");
     if (int rc = wrong_device(m)) return rc;
-    if (m->cfg.has_wo || m->cfg.d_model > 128)
-        return fail(FV_ERR_BAD_SHAPE, "fv_log_prob_static: only the layer-major path (d_model <= 128, no W_O)");
+    if (m->cfg.d_model > 128)
+        return fail(FV_ERR_BAD_SHAPE, "fv_log_prob_static: only the layer-major path (d_model <= 128)");
     const size_t need = fv_logprob_static_need(m->dev, m->cfg.d_model, B);
     if (need > FV_LP_STATIC_BYTES)
         return fail(FV_ERR_BAD_ARG, "fv_log_prob_static: B * N = " + std::to_string((long long)B * m->cfg.n_sites) + " rows need " +

@@ -38,6 +38,7 @@ struct FvLayerDev {
     // fv_logprob.cu: pre-swizzled (SWIZZLE_128B, K-major) bf16 images, copied verbatim into shared memory
     const unsigned char* img_qkv;   // [3d rows x KP]
     const unsigned char* img_ffn;   // per 64-column hidden chunk j: W1_j [64 x KP] | W2_j [d x 64]
+    const unsigned char* img_wo;    // [d rows x KP] (has_wo), same layout
     const unsigned char* img_w1t;   // fv_decode_tc.cu (d = 128): W1 per 128-row M-tile and 64-column K-block, [128 x 64] tiles of 16 KB
 };
 

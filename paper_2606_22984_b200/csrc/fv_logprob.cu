@@ -93,6 +93,17 @@ __device__ __forceinline__ void ln8_to_tile(float4 (&x)[D / 32], const float* __
     }
 }
 
+// The same tile write without the normalisation (operand of the W_O GEMM: the attention output as it is).
+template <int D>
+__device__ __forceinline__ void cvt8_to_tile(const float4 (&x)[D / 32], uint32_t sA, int r, int j) {
+#pragma unroll
+    for (int k = 0; k < D / 32; ++k) {
+        const int f0 = (k * 8 + j) * 4;
+        sts64(sA + (f0 >> 6) * (TM * 128) + umma::sw128_chunk(r, (f0 & 63) >> 3) + (f0 & 7) * 2,
+              pack_bf16(x[k].x, x[k].y), pack_bf16(x[k].z, x[k].w));
+    }
+}
+
 constexpr int RB = 8;             // rows whose loads a warp keeps in flight in the LN prologues
 
 struct LpArgs {
@@ -110,12 +121,18 @@ struct LpArgs {
     const float* bias2;
     const float* ln_g;
     const float* ln_b;
+    int32_t has_wo;                 // attention writes u over q (then lp_qkv_kernel<D, true>: h += W_O u + b_O) instead of h += u
 };
 
 // --------------------------------------------------------------------------------- QKV
-template <int D>
+// WO = true: the optional output projection (PAPER.md:107 bypasses it; reading A8) with the same machinery -- rows of the
+// attention output u (stored over q) -> bf16 A tile, [M,d] x [d,d] against the W_O image, epilogue h += acc + b_O.
+template <int D, bool WO = false>
 __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_constant__ LpArgs a) {
     using G = LpGeo<D>;
+    constexpr int NOUT = WO ? D : G::NQ;                          // output features
+    constexpr int NOUT_CH = WO ? (D <= 256 ? D : 128) : G::NQ_CH;
+    constexpr int W_BYTES = NOUT * G::KP * 2;
     extern __shared__ unsigned char lp_raw[];
     unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(lp_raw) + 1023) & ~(uintptr_t)1023);
     unsigned char* sA = sm;
@@ -133,9 +150,9 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
     const uint32_t tmem = tmem_slot;
     // the layer's whole W_qkv image stays in shared memory for the CTA's lifetime (bulk copies)
     if (tid == 0) {
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(umma::smem_u32(&bar_w)), "r"((uint32_t)G::WQ_BYTES) : "memory");
-        for (int off = 0; off < G::WQ_BYTES; off += 16384) {
-            const uint32_t n = min(16384, G::WQ_BYTES - off);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(umma::smem_u32(&bar_w)), "r"((uint32_t)W_BYTES) : "memory");
+        for (int off = 0; off < W_BYTES; off += 16384) {
+            const uint32_t n = min(16384, W_BYTES - off);
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
                          ::"r"(umma::smem_u32(sW + off)), "l"(a.w_img + off), "r"(n), "r"(umma::smem_u32(&bar_w)) : "memory");
         }
@@ -144,7 +161,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
         for (int i = tid; i < G::A_BYTES / 16; i += LP_THREADS) reinterpret_cast<uint4*>(sA)[i] = make_uint4(0, 0, 0, 0);
         __syncthreads();
     }
-    const uint32_t idesc = umma::make_idesc_bf16(TM, G::NQ_CH);
+    const uint32_t idesc = umma::make_idesc_bf16(TM, NOUT_CH);
     const long long n_tiles = (a.M + TM - 1) / TM;
     uint32_t ph = 0;
     bool w_ready = false;
@@ -160,7 +177,10 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
         for (int ps = 0; ps < RB / 4; ++ps) {
             const int r = warp * RB + ps * 4 + sub;
             const long long gi = tile * TM + r;
-            if (gi < a.M) {
+            if (WO && gi < a.M) {
+#pragma unroll
+                for (int k = 0; k < NV; ++k) x[ps][k] = *reinterpret_cast<const float4*>(a.q + gi * D + (k * 8 + jl) * 4);
+            } else if (gi < a.M) {
                 if (a.layer == 0) {                 // Eq. 15 (l.287-292): x = [tok_emb[s_{t-1}] ; pos_emb[t]]
                     const int t = (int)(gi % a.N);
                     const int tok = t == 0 ? 0 : (a.vocab > 2 ? (int)(uint8_t)a.spins[gi - 1] : (a.spins[gi - 1] > 0 ? 1 : 0));
@@ -192,11 +212,12 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
         for (int ps = 0; ps < RB / 4; ++ps) {
             const int r = warp * RB + ps * 4 + sub;
             const long long gi = tile * TM + r;
-            if (a.layer == 0 && gi < a.M) {
+            if (!WO && a.layer == 0 && gi < a.M) {
 #pragma unroll
                 for (int k = 0; k < NV; ++k) *reinterpret_cast<float4*>(a.h + gi * D + (k * 8 + jl) * 4) = x[ps][k];
             }
-            ln8_to_tile<D>(x[ps], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, jl);
+            if constexpr (WO) cvt8_to_tile<D>(x[ps], sA_u32, r, jl);
+            else ln8_to_tile<D>(x[ps], a.ln_g, a.ln_b, a.ln_eps, sA_u32, r, jl);
         }
         umma::fence_smem_to_async();
         __syncthreads();
@@ -206,13 +227,13 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
             umma::fence_after_sync();
             const uint32_t a0 = umma::smem_u32(sA), w0 = umma::smem_u32(sW);
 #pragma unroll
-            for (int nc = 0; nc < G::NQ / G::NQ_CH; ++nc)
+            for (int nc = 0; nc < NOUT / NOUT_CH; ++nc)
 #pragma unroll
                 for (int kb = 0; kb < G::KB; ++kb)
 #pragma unroll
                     for (int ks = 0; ks < 4; ++ks)
-                        umma::mma_bf16_ss(tmem + nc * G::NQ_CH, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
-                                          umma::make_desc_sw128(w0 + kb * (G::NQ * 128) + nc * (G::NQ_CH * 128) + ks * 32),
+                        umma::mma_bf16_ss(tmem + nc * NOUT_CH, umma::make_desc_sw128(a0 + kb * (TM * 128) + ks * 32),
+                                          umma::make_desc_sw128(w0 + kb * (NOUT * 128) + nc * (NOUT_CH * 128) + ks * 32),
                                           idesc, (kb | ks) != 0);
             umma::commit(&bar_mma);
         }
@@ -233,7 +254,7 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
             const int rB = warp * RPW + lane / LPRW;       // storing: first row, then += RPI
             const int cB = (lane % LPRW) * 16;             //          byte offset inside the row
 #pragma unroll 1
-            for (int pass = 0; pass < 2; ++pass) {
+            for (int pass = 0; pass < (WO ? 1 : 2); ++pass) {
                 const int cb0 = pass == 0 ? 0 : D / 32, cb1 = pass == 0 ? D / 32 : G::NQ / 32;
                 for (int cb = cb0 + (warp >> 2); cb < cb1; cb += NCG) {
                     float v[32];
@@ -262,9 +283,14 @@ __global__ void __launch_bounds__(LP_THREADS, 1) lp_qkv_kernel(const __grid_cons
                     const int row = rB + i * RPI;
                     const long long gi = tile * TM + row;
                     if (gi < a.M) {
-                        const uint4 val = *reinterpret_cast<const uint4*>(sS + row * G::STG_STRIDE + cB);
+                        uint4 val = *reinterpret_cast<const uint4*>(sS + row * G::STG_STRIDE + cB);
                         unsigned char* dst;
-                        if (pass == 0) dst = reinterpret_cast<unsigned char*>(a.q + gi * D);
+                        if constexpr (WO) {              // residual: h += W_O u + b_O
+                            dst = reinterpret_cast<unsigned char*>(a.h + gi * D);
+                            const float4 hv = *reinterpret_cast<const float4*>(dst + cB);
+                            val.x = __float_as_uint(hv.x + __uint_as_float(val.x)); val.y = __float_as_uint(hv.y + __uint_as_float(val.y));
+                            val.z = __float_as_uint(hv.z + __uint_as_float(val.z)); val.w = __float_as_uint(hv.w + __uint_as_float(val.w));
+                        } else if (pass == 0) dst = reinterpret_cast<unsigned char*>(a.q + gi * D);
                         else {
                             const int b = (int)(gi / a.N), t = (int)(gi % a.N);
                             dst = reinterpret_cast<unsigned char*>(a.kv + (((size_t)b * a.NL + a.layer) * a.N + t) * (2 * D));
@@ -304,8 +330,9 @@ __global__ void __launch_bounds__(512) lp_attn_kernel(const __grid_constant__ Lp
         attend_range<D, DH>(a.q + gi * D, a.kv + ((size_t)b * a.NL + a.layer) * a.N * (2 * D), cols, e0, e1, lane, mm, ll, acc);
         if (lane < LPR) {
             const float inv = 1.0f / ll;
-            float* hp = a.h + gi * D + lane * 8;
+            float* hp = (a.has_wo ? a.q : a.h) + gi * D + lane * 8;       // with W_O: u over this row's q (read above)
             float4 h0 = *reinterpret_cast<float4*>(hp), h1 = *reinterpret_cast<float4*>(hp + 4);
+            if (a.has_wo) h0 = h1 = make_float4(0.f, 0.f, 0.f, 0.f);
             h0.x += acc[0] * inv; h0.y += acc[1] * inv; h0.z += acc[2] * inv; h0.w += acc[3] * inv;
             h1.x += acc[4] * inv; h1.y += acc[5] * inv; h1.z += acc[6] * inv; h1.w += acc[7] * inv;
             *reinterpret_cast<float4*>(hp) = h0;
@@ -536,7 +563,7 @@ __global__ void __launch_bounds__(D / 16 * 32, 3) lp_attn_mma_kernel(const __gri
             const int t = t0 + mt * 16 + g + hh * 8;
             const float* hp = a.h + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
 #pragma unroll
-            for (int x = 0; x < 2; ++x) hres[mt][hh][x] = t < a.N ? *reinterpret_cast<const float2*>(hp + x * 8) : make_float2(0.f, 0.f);
+            for (int x = 0; x < 2; ++x) hres[mt][hh][x] = (t < a.N && !a.has_wo) ? *reinterpret_cast<const float2*>(hp + x * 8) : make_float2(0.f, 0.f);
         }
 #pragma unroll
     for (int mt = 0; mt < 2; ++mt)
@@ -548,7 +575,8 @@ __global__ void __launch_bounds__(D / 16 * 32, 3) lp_attn_mma_kernel(const __gri
             const int t = t0 + mt * 16 + g + hh * 8;
             if (t < a.N && l > 0.f) {
                 const float inv = 1.0f / l;
-                float* hp = a.h + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
+                // with W_O the output u replaces this warp's own q elements (its Q fragments were read at the start)
+                float* hp = (a.has_wo ? a.q : a.h) + ((long long)b * a.N + t) * D + head * 16 + 2 * c;
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
                     float2 hv = hres[mt][hh][x];
@@ -914,12 +942,14 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
     {
         cudaError_t e = fv_smem_attr((const void*)lp_qkv_kernel<D>, G::QKV_SMEM);
         if (e == cudaSuccess) e = fv_smem_attr((const void*)lp_ffn_kernel<D>, G::FFN_SMEM);
+        if (e == cudaSuccess && m.has_wo) e = fv_smem_attr((const void*)lp_qkv_kernel<D, true>, G::QKV_SMEM);
         if (e == cudaSuccess) e = fv_smem_attr((const void*)lp_attn_mma_kernel<D>, att_smem);
         if (e != cudaSuccess) return e;
     }
     LpArgs a{};
     a.B = B; a.N = m.n_sites; a.NL = m.n_layers; a.d_token = m.d_token; a.ln2_style = m.ln2_style; a.ln_eps = m.ln_eps;
     a.vocab = m.vocab;
+    a.has_wo = m.has_wo;
     a.M = (long long)B * m.n_sites;
     a.spins = spins; a.h = m.lp_h; a.q = m.lp_q; a.kv = m.kv; a.tok_emb = m.tok_emb; a.posemb = m.posemb;
     const long long n_tiles = (a.M + TM - 1) / TM;
@@ -942,6 +972,12 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
                                                                                                 rows_per_cta);
         }
         fv_prof_end(FV_K_LP_ATTN, s);
+        if (m.has_wo) {                               // h += W_O u + b_O (u sits where q was)
+            a.w_img = L.img_wo; a.bias = L.bo;
+            fv_prof_begin(FV_K_LP_QKV, s);
+            lp_qkv_kernel<D, true><<<grid, LP_THREADS, G::QKV_SMEM, s>>>(a);
+            fv_prof_end(FV_K_LP_QKV, s);
+        }
         a.w_img = L.img_ffn; a.bias = L.b1; a.bias2 = L.b2; a.ln_g = L.ln2_g; a.ln_b = L.ln2_b;
         fv_prof_begin(FV_K_LP_FFN, s);
         lp_ffn_kernel<D><<<grid_ffn, FFN_THREADS, G::FFN_SMEM, s>>>(a);
@@ -960,8 +996,8 @@ cudaError_t launch_lp(const FvModelDev& m, int B, const int8_t* spins, float* lo
 // cudaErrorNotSupported otherwise (the caller then uses the chunked teacher-forcing kernel).
 cudaError_t fv_launch_logprob_tc(const FvModelDev& m, int d_model, int d_head, int B, const int8_t* spins, float* logq,
                                  float* cond_p, int n_sms, int* n_launches, cudaStream_t s) {
-    if (m.has_wo || !m.lp_h) return cudaErrorNotSupported;
-    *n_launches = 3 * m.n_layers + 1;
+    if (!m.lp_h) return cudaErrorNotSupported;
+    *n_launches = (m.has_wo ? 4 : 3) * m.n_layers + 1;
     switch (d_model * 1000 + d_head) {
         case 32016: return launch_lp<32, 16>(m, B, spins, logq, cond_p, n_sms, s);
         case 64016: return launch_lp<64, 16>(m, B, spins, logq, cond_p, n_sms, s);

@@ -63,8 +63,15 @@ def test_static_workspace_limit_and_shapes():
     got, _ = model.log_prob_static(spins[:fit].contiguous(), lq[:fit])              # exactly at the limit
     assert torch.equal(got, ref)
     model.close()
-    wo = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2, has_wo=1)
-    model = make(wo, 4)
+    wide = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2, d_model=256, n_heads=4)
+    model = make(wide, 4)                                                           # d = 256 has no layer-major path
     with pytest.raises(fv.FlashVanError, match="layer-major"):
-        model.log_prob_static(torch.from_numpy(W.make_spins(wo, 4)).cuda(), torch.empty(4, device="cuda"))
+        model.log_prob_static(torch.from_numpy(W.make_spins(wide, 4)).cuda(), torch.empty(4, device="cuda"))
+    model.close()
+    wo = dataclasses.replace(W.CONFIGS["cfg2"], L=6, n_sites=36, window=5, n_layers=2, has_wo=1)
+    model = make(wo, 4)                                                             # W_O: the extra tcgen05 GEMM per layer
+    spins = torch.from_numpy(W.make_spins(wo, 4)).cuda()
+    ref, _ = model.log_prob(spins)
+    got, _ = model.log_prob_static(spins, torch.empty(4, device="cuda"))
+    assert torch.equal(got, ref)
     model.close()
