@@ -574,17 +574,24 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                             for (int j = 0; j < 4; ++j) { acc[2 * j] = bf_lo(vw[j]); acc[2 * j + 1] = bf_hi(vw[j]); }
                         }
                     }
-                    // row group g < FV_DIRECT_MAX requests the step's g-th isolated row now and uses it after the ring's rows
-                    // (written by this CTA in an earlier step, plain stores; barriers since)
-                    uint4 dk = make_uint4(0u, 0u, 0u, 0u), dv = dk;
-                    int dpos = -1;
+                    // The step's isolated rows, RPID per load: row group g takes row b0 + g.  The first set is requested now and
+                    // used after the ring's rows; further sets (lattice edges, 3D masks) are loaded then.  (Rows this CTA wrote
+                    // in an earlier step with plain stores; barriers since.)
+                    constexpr int RPID = 32 / LPRS;
+                    auto dir_load = [&](int b0, uint4& k4, uint4& v4) {
+                        int dpos = -1;
 #pragma unroll
-                    for (int i = 0; i < FV_DIRECT_MAX; ++i) if (rgs == i) dpos = dir_pos[i];
-                    if (dpos >= 0) {
-                        const __nv_bfloat16* dp = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + dpos) * (2 * D) + sp * DS + subs * 8;
-                        dk = *reinterpret_cast<const uint4*>(dp);
-                        dv = *reinterpret_cast<const uint4*>(dp + D);
-                    }
+                        for (int i = 0; i < RPID; ++i) if (rgs == i && b0 + i < FV_DIRECT_MAX) dpos = dir_pos[b0 + i < FV_DIRECT_MAX ? b0 + i : 0];
+                        k4 = v4 = make_uint4(0u, 0u, 0u, 0u);
+                        if (dpos >= 0) {
+                            const __nv_bfloat16* dp = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + dpos) * (2 * D) + sp * DS + subs * 8;
+                            k4 = *reinterpret_cast<const uint4*>(dp);
+                            v4 = *reinterpret_cast<const uint4*>(dp + D);
+                        }
+                        return dpos >= 0;
+                    };
+                    uint4 dk, dv;
+                    const bool dok = dir_load(0, dk, dv);
                     for (int c = 0; c < nch; ++c) {
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
                         const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
@@ -595,7 +602,14 @@ fv_decode_kernel(const __grid_constant__ FvModelDev m, const __grid_constant__ F
                         ring_release_dep(rc, slot, lane, 1, __float_as_uint(ll) ^ __float_as_uint(acc[0]) ^ __float_as_uint(acc[2]) ^
                                                                 __float_as_uint(acc[4]) ^ __float_as_uint(acc[6]));
                     }
-                    if (dir_pos[0] >= 0) attend_direct<DH>(dk, dv, dpos >= 0, q, mm, ll, acc);
+                    if (dir_pos[0] >= 0) attend_direct<DH>(dk, dv, dok, q, mm, ll, acc);
+#pragma unroll
+                    for (int b0 = RPID; b0 < FV_DIRECT_MAX; b0 += RPID) {
+                        if (dir_pos[b0] < 0) break;
+                        uint4 k4, v4;
+                        const bool ok4 = dir_load(b0, k4, v4);
+                        attend_direct<DH>(k4, v4, ok4, q, mm, ll, acc);
+                    }
 #pragma unroll
                     for (int o = LPRS; o < 32; o <<= 1) {      // merge the row groups of the warp
                         const float m2 = __shfl_xor_sync(0xffffffffu, mm, o);

@@ -19,7 +19,7 @@ constexpr int FV_LP_HC = 64;
 #ifndef FV_DEC_CH128
 #define FV_DEC_CH128 16
 #endif
-#define FV_DIRECT_MAX 2
+#define FV_DIRECT_MAX 6
 constexpr int fv_ring_ch(int d_model) { return d_model >= 256 ? 8 : (d_model >= 128 ? FV_DEC_CH128 : 16); }
 
 // Per-layer device pointers.  GEMM weights are bf16, pre-packed at fv_create_model time into
