@@ -173,21 +173,22 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
             auto stage_plan = [&](int t) {
                 Plan p;
                 if (t >= N) { p.nch = p.nn = p.nruns = 0; p.cptr = nullptr; p.rptr = nullptr; return p; }
-                const int cp0 = __ldg(m.chunk_ptr + t);
-                p.nch = __ldg(m.chunk_ptr + t + 1) - cp0;
-                p.nn = __ldg(m.mask_rowptr + t + 1) - 1 - __ldg(m.mask_rowptr + t);
-                const int rp0 = __ldg(m.chunk_run_ptr + cp0);
-                p.nruns = __ldg(m.chunk_run_ptr + cp0 + p.nch) - rp0;
+                // the plan without the step's isolated rows (fv_internal.h: d_*): those the attention warps load themselves
+                const int cp0 = __ldg(m.d_chunk_ptr + t);
+                p.nch = __ldg(m.d_chunk_ptr + t + 1) - cp0;
+                p.nn = __ldg(m.d_nn + t);
+                const int rp0 = __ldg(m.d_chunk_run_ptr + cp0);
+                p.nruns = __ldg(m.d_chunk_run_ptr + cp0 + p.nch) - rp0;
                 int32_t* tc = tab_c + (t & 1) * TAB_C;
                 int2* tr = tab_r + (t & 1) * TAB_R;
                 __syncwarp();
                 if (p.nch + 1 <= TAB_C && p.nruns <= TAB_R) {
-                    for (int i = lane; i <= p.nch; i += 32) tc[i] = __ldg(m.chunk_run_ptr + cp0 + i) - rp0;
-                    for (int i = lane; i < p.nruns; i += 32) tr[i] = __ldg(m.runs + rp0 + i);
+                    for (int i = lane; i <= p.nch; i += 32) tc[i] = __ldg(m.d_chunk_run_ptr + cp0 + i) - rp0;
+                    for (int i = lane; i < p.nruns; i += 32) tr[i] = __ldg(m.d_runs + rp0 + i);
                     __syncwarp();
                     p.cptr = tc; p.rptr = tr;
                 } else {
-                    p.cptr = m.chunk_run_ptr + cp0; p.rptr = m.runs;
+                    p.cptr = m.d_chunk_run_ptr + cp0; p.rptr = m.d_runs;
                 }
                 return p;
             };
@@ -312,7 +313,10 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
         if (tid < R) { sh_tok[tid] = 0; sh_logq[tid] = 0.0; }
         for (int t = 0; t < N; ++t) {
             const int me0 = __ldg(m.mask_rowptr + t);
-            const int nn = __ldg(m.mask_rowptr + t + 1) - 1 - me0;
+            const int nn = __ldg(m.d_nn + t);                        // rows that come through the ring
+            int dir_pos[FV_DIRECT_MAX];                              // isolated key positions, loaded straight from the pool
+#pragma unroll
+            for (int i = 0; i < FV_DIRECT_MAX; ++i) dir_pos[i] = __ldg(m.d_dir + (size_t)t * FV_DIRECT_MAX + i);
             const int nch = (nn + CH - 1) / CH;
             if (tid < R) sh_u[tid] = tid < n_own ? __ldg(a.uniforms + (size_t)(b_first + tid) * N + t) : 2.f;
             cbar();
@@ -380,6 +384,23 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
                             for (int j = 0; j < 8; ++j) acc[j] = __bfloat162float(kvrow[D + sub * 8 + j]);
                         }
                     }
+                    // isolated rows of the step, one per row group and load; the first set is requested before the ring's rows
+                    constexpr int RPID = 32 / LPR;
+                    auto dir_load = [&](int b0, uint4& k4, uint4& v4) {
+                        int dpos = -1;
+#pragma unroll
+                        for (int i = 0; i < RPID; ++i) if (rg == i && b0 + i < FV_DIRECT_MAX) dpos = dir_pos[b0 + i < FV_DIRECT_MAX ? b0 + i : 0];
+                        if (sp != 0) dpos = -1;
+                        k4 = v4 = make_uint4(0u, 0u, 0u, 0u);
+                        if (dpos >= 0) {
+                            const __nv_bfloat16* dp = m.kv_s + (((size_t)(b_first + r) * NL + l) * m.kv_rows + dpos) * (2 * D) + sub * 8;
+                            k4 = *reinterpret_cast<const uint4*>(dp);
+                            v4 = *reinterpret_cast<const uint4*>(dp + D);
+                        }
+                        return dpos >= 0;
+                    };
+                    uint4 dk, dv;
+                    const bool dok = dir_load(0, dk, dv);
                     for (int c = sp; c < nch; c += NSPLIT) {
                         const int kr = r / GR, nk = min(GR, n_own - kr * GR);
                         const uint32_t sq = seq_base + (uint32_t)(kr * GR * nch + c * nk + (r - kr * GR));
@@ -390,6 +411,14 @@ fv_decode_tc_kernel(const __grid_constant__ FvModelDev m, const __grid_constant_
                         // ll, the V words fed acc[0..1] / [2..3] / [4..5] / [6..7]
                         ring_release_dep(rc, slot, lane, 1, __float_as_uint(ll) ^ __float_as_uint(acc[0]) ^ __float_as_uint(acc[2]) ^
                                                                 __float_as_uint(acc[4]) ^ __float_as_uint(acc[6]));
+                    }
+                    if (dir_pos[0] >= 0) attend_direct<DH>(dk, dv, dok, q, mm, ll, acc);
+#pragma unroll
+                    for (int b0 = RPID; b0 < FV_DIRECT_MAX; b0 += RPID) {
+                        if (dir_pos[b0] < 0) break;
+                        uint4 k4, v4;
+                        const bool ok4 = dir_load(b0, k4, v4);
+                        attend_direct<DH>(k4, v4, ok4, q, mm, ll, acc);
                     }
 #pragma unroll
                     for (int o = LPR; o < 32; o <<= 1) {       // merge the row groups of the warp
