@@ -374,6 +374,27 @@ def test_random_csr_masks(density, d_model, n_heads):
     model.close()
 
 
+@pytest.mark.parametrize("kind,B", [("ring", 21), ("ring", 150), ("tc", 300)])
+def test_isolated_rows_are_loaded_directly(kind, B, monkeypatch):
+    """Copy plan of the streaming samplers: up to six ISOLATED key positions per step bypass the ring (the attention warps
+    load them from the pool), the rest goes through it.  Rows with 0, 1, ..., 9 isolated keys next to a run of 20, with and
+    without a ragged tail, on the mma.sync kernel (8 and 16+ rows per CTA) and the tcgen05 kernel."""
+    N = 120
+    w = dataclasses.replace(W.CONFIGS["cfg5"], L=N, n_sites=N, n_layers=2)
+    rows = []
+    for t in range(N):
+        run = list(range(max(0, t - 20 - (t % 3)), t))                 # a run whose length is not a multiple of 16
+        far = [p for p in range(0, max(0, t - 40), 4)][: t % 10]        # isolated keys: every fourth position, 0..9 of them
+        rows.append(np.array(sorted(set(far + run + [t])), dtype=np.int32))
+    rp = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int32)
+    col = np.concatenate(rows).astype(np.int32)
+    monkeypatch.setenv("FLASHVAN_DECODE", kind)
+    model, weights, posemb, rp, col = build(w, B, mask=(rp, col))
+    assert model.sampler_kind(B) == ("ring-tc" if kind == "tc" else "ring")
+    check_sample(w, model, weights, posemb, rp, col, W.make_uniforms(w, B, seed=17))
+    model.close()
+
+
 @pytest.mark.parametrize("periodic", [False, True])
 def test_markov_boundary_mask_from_the_library(periodic):
     """The paper's own mask: ordered Markov boundary of a 12 x 12 lattice built by
