@@ -344,6 +344,26 @@ def test_sample_is_reproducible_across_fresh_models():
         model.close()
 
 
+@pytest.mark.parametrize("name", ["cfg5", "cfg4"])
+def test_full_size_sample_is_reproducible(name):
+    """The same at BASELINE size, in bench.py's launch geometry (cfg5: mma.sync sampler, 7 samples per CTA; cfg4: tcgen05
+    sampler, 28 per CTA): ring slots are released through a data dependency instead of a proxy fence (fv_ring.cuh,
+    ring_release_dep) -- a refill overtaking reads would show as run-to-run differences at this size first."""
+    w = W.CONFIGS[name]
+    inp = W.make_all(w)
+    u = dev(inp["uniforms"])
+    ref = None
+    for it in range(3):
+        model = fv.create_model(w, inp["weights"], inp["mask_rowptr"], inp["mask_col"], inp["posemb"], w.batch)
+        junk = torch.randn(64 << 20, device="cuda")
+        del junk
+        out = [x.clone() for x in model.sample(u, want_cond_p=True)]
+        model.close()
+        if ref is None:
+            ref = out
+        assert all(torch.equal(x, y) for x, y in zip(out, ref)), f"run {it} differs"
+
+
 @pytest.mark.parametrize("N", [1, 2, 3, 17])
 def test_tiny_sequences(N):
     """Degenerate lengths: N = 1 (only the start token), N = 2, 3 and a ragged 17; full causal mask,
