@@ -13,6 +13,12 @@
 // the host plan), W_o, W_1, W_2.  The 16 COMPUTE warps read K/V and the mma.sync A fragments from
 // shared memory.  Row t itself is attended from the shared memory of the step that produced it
 // (rounded to bf16 exactly as the pool stores it).
+// What paces the kernel is the latency chain "consumer frees slots -> producer round -> copies land" (DESIGN.md 6.1,
+// profiles/r03_fv_sample.md), so: weight chunks travel two per bulk copy; isolated key rows (runs of one row) bypass the ring
+// and are loaded by the attention warps (plan d_* of fv_internal.h); the producer maps chunk -> (sample, chunk) without
+// integer divisions; slots are released through a data dependency instead of a proxy fence (ring_release_dep); the two
+// warps of a sample split its query row by heads (no partial results, no combine phase); a layer's small parameters are
+// staged in shared memory by warps that would otherwise wait.
 // Optional (FLASHVAN_DECODE=cluster): 2-CTA clusters in which each CTA streams only its half of
 // W_1/W_2 and applies it to the rows of both CTAs, exchanging LN2 rows and partial sums through
 // distributed shared memory (correct, measured slower: DESIGN.md 6.1).
